@@ -1,0 +1,233 @@
+"""
+FDAS oracle -- TEST INFRASTRUCTURE ONLY.  Never imported by the product path
+(`paper_1804_05335_b200/`); only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / `--impl reference` legs may use it.  It shares no code, tables or
+constants with the CUDA path.
+
+What it computes (fp64 throughout), each function citing the passage it follows:
+
+  * template taps  h_z[d]  -- the "predicted normalised Fourier response" of
+    PAPER.md:65 (section 2).  The paper cites the formula (Ransom et al. 2002) but does
+    not print it; reading R1 defines it as the response, at bin offset d from
+    the mid-observation frequency, of a unit-amplitude tone drifting linearly by z bins:
+        h_z(d) = integral_0^1 exp( 2 pi i [ -d u + z (u^2 - u)/2 ] ) du
+    evaluated HERE BY NUMERICAL QUADRATURE of that integral (the CUDA path uses the
+    Fresnel closed form instead, so the two share no formula path).
+  * the correlation of eq. 3 by direct summation (C, oracle/fdas_oracle.c),
+  * Fourier power and interbinning, eq. 4 applied to the
+    correlated complex amplitudes.
+
+Pins (tests/test_oracle_pins.py): closed form via scipy's Fresnel integrals, the z=0
+sinc/delta special case, brute-force time-domain chirp + DFT, injected-chirp peak,
+reversal / shift / linearity invariants, noise statistics, the paper's printed
+interbinning losses, fp64 FFT overlap-save at two segment lengths,
+and a pure-Python triple loop on tiny inputs.  No function here is "parity unpinned".
+"""
+from __future__ import annotations
+
+import ctypes
+import functools
+import math
+
+import numpy as np
+
+from . import build as _build
+
+# --------------------------------------------------------------------------------------
+# template bank (readings R4, R9; BASELINE.json configs: "half-width ceil(|z|/2)+16")
+# --------------------------------------------------------------------------------------
+
+
+def bank_z(zmax: float, dz: float) -> np.ndarray:
+    """Trial z values, ascending: z_k = -zmax + k*dz, k = 0..K-1 (reading R9)."""
+    nhalf = int(round(zmax / dz))
+    if abs(nhalf * dz - zmax) > 1e-9 * max(1.0, abs(zmax)):
+        raise ValueError("zmax/dz must be an integer")
+    return np.array([-zmax + k * dz for k in range(2 * nhalf + 1)], dtype=np.float64)
+
+
+def halfwidth(z: float) -> int:
+    """Per-template half-width m_z = ceil(|z|/2) + 16 bins (BASELINE.json config 1)."""
+    return int(math.ceil(abs(z) / 2.0 - 1e-12)) + 16
+
+
+@functools.lru_cache(maxsize=None)
+def _gauss_legendre(n: int):
+    x, w = np.polynomial.legendre.leggauss(n)
+    return x, w
+
+
+def response(z: float, d) -> np.ndarray:
+    """
+    h_z(d) for real bin offsets d (array-like), by composite Gauss-Legendre quadrature of
+        integral_0^1 exp(2 pi i [ -d u + z (u^2 - u)/2 ]) du        (reading R1)
+    The panel count is chosen so the phase advances by at most ~pi/4 per panel; with 12
+    nodes per panel the quadrature error is far below 1e-15.
+    """
+    d = np.atleast_1d(np.asarray(d, dtype=np.float64))
+    nodes, weights = _gauss_legendre(12)
+    # |d phase/du| <= 2 pi (|d| + |z|/2)
+    rate = float(np.max(np.abs(d))) + abs(z) / 2.0 + 1.0
+    npanel = int(math.ceil(8.0 * rate))
+    edges = np.linspace(0.0, 1.0, npanel + 1)
+    half = 0.5 * (edges[1:] - edges[:-1])
+    mid = 0.5 * (edges[1:] + edges[:-1])
+    u = (mid[:, None] + half[:, None] * nodes[None, :]).ravel()          # all nodes
+    w = (half[:, None] * weights[None, :]).ravel()                       # all weights
+    out = np.empty(d.shape, dtype=np.complex128)
+    chirp = z * (u * u - u) / 2.0
+    for i, di in enumerate(d):
+        phase = 2.0 * np.pi * (-di * u + chirp)
+        out[i] = np.sum(w * np.cos(phase)) + 1j * np.sum(w * np.sin(phase))
+    return out
+
+
+@functools.lru_cache(maxsize=None)
+def _taps_cached(z: float, m: int) -> np.ndarray:
+    t = response(z, np.arange(-m, m + 1, dtype=np.float64))
+    t.setflags(write=False)
+    return t
+
+
+def taps(z: float, m: int | None = None) -> np.ndarray:
+    """Taps h_z[d], d = -m..+m (complex128, index d+m); m defaults to halfwidth(z)."""
+    if m is None:
+        m = halfwidth(z)
+    return _taps_cached(float(z), int(m))
+
+
+# --------------------------------------------------------------------------------------
+# correlation, eq. 3 -- C direct sum
+# --------------------------------------------------------------------------------------
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(_build.build())
+        i64, i32, vp = ctypes.c_int64, ctypes.c_int32, ctypes.c_void_p
+        lib.fdas_oracle_correlate.argtypes = [vp, i64, vp, i32, i64, i64, vp]
+        lib.fdas_oracle_correlate.restype = None
+        lib.fdas_oracle_correlate_at.argtypes = [vp, i64, vp, i32, vp, i64, vp]
+        lib.fdas_oracle_correlate_at.restype = None
+        lib.fdas_oracle_threads.restype = i32
+        _lib = lib
+    return _lib
+
+
+def threads() -> int:
+    """OpenMP threads the C direct sum will use."""
+    return int(_load().fdas_oracle_threads())
+
+
+def _as_c64(spectrum) -> np.ndarray:
+    a = np.ascontiguousarray(spectrum, dtype=np.complex64)
+    if a.ndim != 1:
+        raise ValueError("spectrum must be 1-D")
+    return a
+
+
+def correlate(spectrum, h: np.ndarray, r_begin: int = 0, r_count: int | None = None) -> np.ndarray:
+    """y[r] = sum_d A[r+d] conj(h[d]) for r in [r_begin, r_begin+r_count); zero extension (R7)."""
+    a = _as_c64(spectrum)
+    h = np.ascontiguousarray(h, dtype=np.complex128)
+    m = (h.size - 1) // 2
+    assert h.size == 2 * m + 1
+    if r_count is None:
+        r_count = a.size - r_begin
+    y = np.empty(r_count, dtype=np.complex128)
+    _load().fdas_oracle_correlate(a.ctypes.data, a.size, h.ctypes.data, m,
+                                  int(r_begin), int(r_count), y.ctypes.data)
+    return y
+
+
+def correlate_at(spectrum, h: np.ndarray, cols) -> np.ndarray:
+    """y at the listed columns only (sampled checks at full size)."""
+    a = _as_c64(spectrum)
+    h = np.ascontiguousarray(h, dtype=np.complex128)
+    m = (h.size - 1) // 2
+    cols = np.ascontiguousarray(cols, dtype=np.int64)
+    y = np.empty(cols.size, dtype=np.complex128)
+    _load().fdas_oracle_correlate_at(a.ctypes.data, a.size, h.ctypes.data, m,
+                                     cols.ctypes.data, cols.size, y.ctypes.data)
+    return y
+
+
+def correlate_numpy(spectrum, h: np.ndarray) -> np.ndarray:
+    """Same sum as `correlate` over all N columns, written with numpy slices (cross-check of the C)."""
+    a = _as_c64(spectrum).astype(np.complex128)
+    n = a.size
+    m = (h.size - 1) // 2
+    y = np.zeros(n, dtype=np.complex128)
+    for d in range(-m, m + 1):
+        lo, hi = max(0, -d), min(n, n - d)          # r with 0 <= r+d < n
+        if hi > lo:
+            y[lo:hi] += a[lo + d:hi + d] * np.conj(h[d + m])
+    return y
+
+
+# --------------------------------------------------------------------------------------
+# power and interbinning
+# --------------------------------------------------------------------------------------
+
+INTERBIN_SCALE = math.pi / 4.0            # eq. 4
+
+
+def power_from_amplitudes(y: np.ndarray) -> np.ndarray:
+    """P = |y|^2."""
+    return y.real * y.real + y.imag * y.imag
+
+
+def interbin_from_amplitudes(y_ext: np.ndarray) -> np.ndarray:
+    """
+    y_ext = y[0..N] (N+1 amplitudes, y[N] from the zero-extended sum, reading R7).
+    Returns 2N powers: P[2r] = |y[r]|^2, P[2r+1] = |(pi/4)(y[r] - y[r+1])|^2
+    -- eq. 4 applied to the correlated amplitudes,
+    interleaved in natural frequency order (reading R8).
+    """
+    n = y_ext.size - 1
+    out = np.empty(2 * n, dtype=np.float64)
+    out[0::2] = power_from_amplitudes(y_ext[:n])
+    half = INTERBIN_SCALE * (y_ext[:n] - y_ext[1:])
+    out[1::2] = power_from_amplitudes(half)
+    return out
+
+
+def plane_row(spectrum, z: float, interbin: bool = False, m: int | None = None) -> np.ndarray:
+    """One row of the f-fdot plane (float64): N columns, or 2N interbinned."""
+    a = _as_c64(spectrum)
+    h = taps(z, m)
+    if interbin:
+        return interbin_from_amplitudes(correlate(a, h, 0, a.size + 1))
+    return power_from_amplitudes(correlate(a, h, 0, a.size))
+
+
+def plane(spectrum, zmax: float, dz: float, interbin: bool = False) -> np.ndarray:
+    """Whole plane, K rows ascending in z (reading R9).  For sizes that fit in memory."""
+    zs = bank_z(zmax, dz)
+    return np.stack([plane_row(spectrum, z, interbin) for z in zs])
+
+
+def plane_cells(spectrum, z: float, cols, interbin: bool = False) -> np.ndarray:
+    """
+    Sampled cells of one row.  `cols` are plane column indices (0..N-1, or 0..2N-1 when
+    interbinned: even 2r -> bin r, odd 2r+1 -> bin r+1/2).
+    """
+    a = _as_c64(spectrum)
+    h = taps(z)
+    cols = np.asarray(cols, dtype=np.int64)
+    if not interbin:
+        return power_from_amplitudes(correlate_at(a, h, cols))
+    r = cols // 2
+    y0 = correlate_at(a, h, r)
+    y1 = correlate_at(a, h, r + 1)
+    odd = (cols % 2) == 1
+    return np.where(odd, power_from_amplitudes(INTERBIN_SCALE * (y0 - y1)),
+                    power_from_amplitudes(y0))
+
+
+def cmacs(n: int, zmax: float, dz: float) -> int:
+    """Complex multiply-accumulates of the direct sum for one spectrum: N * sum_z (2 m_z + 1)."""
+    return int(n) * int(sum(2 * halfwidth(z) + 1 for z in bank_z(zmax, dz)))

@@ -1,0 +1,149 @@
+/*
+ * fdas.h -- C ABI of the B200-native FDAS correlation hot path (arXiv:1804.05335).
+ *
+ * The library computes the f-fdot power plane of the paper's "correlation technique":
+ * the overlap-save convolution of a complex Fourier spectrum with a bank of
+ * per-trial-z Fourier-domain FIR templates, followed by |.|^2 (optionally interbinned).
+ * Citations are to /root/reference/PAPER.md (line numbers) and to DESIGN.md readings (Rn).
+ *
+ *   result (eq. 3):
+ *       y_z[r] = sum_{d=-m_z}^{+m_z} A[r+d] * conj(h_z[d]),  A[j] := 0 outside [0, nbins)
+ *       P[z][r] = |y_z[r]|^2
+ *   method (PAPER.md:75-77, :87 Fig. 1, :105, :129-131): per overlapping segment of
+ *       `seglen` bins: forward FFT, pointwise multiply by each template's precomputed
+ *       FFT, inverse FFT, discard the contaminated edges, power, contiguous store.
+ *   interbinning (PAPER.md:81-83 eq. 4, :89, :95), applied to the correlated amplitudes:
+ *       P[z][2r] = |y_z[r]|^2,  P[z][2r+1] = |(pi/4)(y_z[r] - y_z[r+1])|^2
+ *
+ * All entry points are plain C, take plain pointers and sizes, return a status code and
+ * never throw or abort.  "device" pointers are CUDA device pointers on the device that
+ * was current when the plan was created; "host" pointers are ordinary host memory.
+ * `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ * There is no CPU fallback anywhere in this library.
+ */
+#ifndef FDAS_H_
+#define FDAS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fdas_plan fdas_plan; /* opaque; created/destroyed by the library */
+
+typedef enum fdas_status {
+    FDAS_OK = 0,
+    FDAS_ERR_INVALID_ARG = 1, /* null pointer, nbins <= 0, zmax < 0, dz <= 0, zmax/dz not an integer      */
+    FDAS_ERR_UNSUPPORTED = 2, /* seglen not in {1024, 2048, 4096, 8192}, or too short for the bank's overlap */
+    FDAS_ERR_NOT_READY = 3,   /* fdas_execute before fdas_make_templates                                    */
+    FDAS_ERR_ALIGNMENT = 4,   /* device pointer not 16-byte aligned                                         */
+    FDAS_ERR_CUDA = 5,        /* a CUDA runtime call failed; see fdas_last_error()                          */
+    FDAS_ERR_NOMEM = 6        /* host or device allocation failed                                           */
+} fdas_status;
+
+/* Geometry of a plan (filled by fdas_plan_info). */
+typedef struct fdas_info {
+    int64_t nbins;        /* N: complex bins in the spectrum                                         */
+    int64_t ncols;        /* plane columns: N, or 2N when interbinned                                */
+    int64_t row_stride;   /* floats between consecutive rows of the plane (= ncols)                  */
+    int64_t nseg;         /* overlap-save segments: ceil(N / useful)                                 */
+    int64_t plane_bytes;  /* ntemplates * ncols * 4                                                  */
+    double zmax, dz;      /* bank: z_k = -zmax + k*dz, k = 0..ntemplates-1 (ascending, R9)           */
+    int32_t ntemplates;   /* K = 2*zmax/dz + 1                                                       */
+    int32_t seglen;       /* L: segment FFT length                                                   */
+    int32_t halfwidth;    /* m = ceil(zmax/2) + 16: half-width of the widest template (R4)           */
+    int32_t overlap;      /* bins discarded at each end of a segment (>= m, +1 with interbinning;
+                             rounded up to a multiple of 32 so segment loads/stores stay 128B-aligned) */
+    int32_t useful;       /* B = L - 2*overlap useful output bins per segment                        */
+    int32_t interbin;     /* 0/1                                                                     */
+    int32_t npairs;       /* (K+1)/2 template slots processed by the kernel (+-z share one slot)      */
+    int32_t threads;      /* threads per CTA of the fused kernel                                     */
+    int32_t grid;         /* CTAs launched by fdas_execute (persistent; multiple of the SM count)    */
+    int32_t ctas_per_sm;  /* resident CTAs per SM the grid was sized for                             */
+    int32_t smem_bytes;   /* dynamic shared memory per CTA                                           */
+    int32_t regs;         /* registers per thread of the fused kernel                                */
+    int32_t sm_count;     /* SMs on the device                                                       */
+    int32_t reserved;
+} fdas_info;
+
+/*
+ * Create a plan for spectra of `nbins` complex64 bins and the template bank
+ * z = -zmax .. +zmax step dz ("K acceleration templates"; BASELINE.json),
+ * each template of half-width ceil(|z|/2)+16 bins (R4), segment FFT length `seglen`
+ * ("blocks of length L"), with or without interbinning.
+ * Allocates the plan-owned device memory (taps, template spectra, twiddle table).
+ * *out is set to NULL on failure.
+ */
+fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double dz,
+                             int32_t seglen, int32_t interbin);
+
+/*
+ * Generate the template bank on the device, enqueued on `stream` (no host sync):
+ *  a0  taps h_z[d], |d| <= m_z: the "predicted normalised Fourier response",
+ *      Fresnel-integral closed form of  int_0^1 exp(2 pi i[-d u + z(u^2-u)/2]) du  (R1), fp64;
+ *  a1  template spectra H_z = (1/L) DFT_L(g_z), g_z[j mod L] = conj(h_z[-j]) -- the filter
+ *      "centered at bin zero", halves at both ends of an L-array, zeros between
+ *      (PAPER.md:77, :87), evaluated in fp64, stored as complex64 in the fused kernel's
+ *      un-permuted FFT order; only z <= 0 is stored, +z is applied as
+ *      the complex conjugate.  1/L of eq. 6 is folded in (R6).
+ */
+fdas_status fdas_make_templates(fdas_plan *plan, void *stream);
+
+/*
+ * Compute the f-fdot plane of one spectrum: one fused kernel launch on `stream`.
+ *   d_spectrum : device, nbins x {float re, float im} (complex64), 16-byte aligned; read only.
+ *   d_plane    : device, ntemplates x ncols float32, row-major, 16-byte aligned; every
+ *                element is written.  Row k <-> z_k ascending; column r <-> bin r
+ *                (interbinned: column 2r <-> bin r, 2r+1 <-> bin r + 1/2).
+ * Allocates nothing, never synchronises the host, may be called repeatedly (e.g. once per
+ * spectrum of a batch on one stream).  Caller owns both buffers.
+ */
+fdas_status fdas_execute(fdas_plan *plan, void *stream, const void *d_spectrum, float *d_plane);
+
+/*
+ * End-to-end convenience for HOST buffers: copies `h_spectrum` (nbins complex64) to a
+ * plan-owned device buffer, runs fdas_execute, copies the plane back to `h_plane`
+ * (ntemplates x ncols float32) and synchronises `stream`.  Device staging buffers are
+ * allocated on first use and freed by fdas_destroy.  Pinned host memory is recommended.
+ */
+fdas_status fdas_execute_host(fdas_plan *plan, void *stream, const void *h_spectrum, float *h_plane);
+
+/* Free the plan and everything it owns.  fdas_destroy(NULL) is a no-op returning FDAS_OK. */
+fdas_status fdas_destroy(fdas_plan *plan);
+
+/* ---- introspection for harnesses and tests (not on the hot path) ---- */
+
+fdas_status fdas_plan_info(const fdas_plan *plan, fdas_info *out);
+
+/*
+ * Copy template k's taps to the host (synchronises): host_re_im receives
+ * 2*(2*halfwidth_k+1) doubles, interleaved (re, im), index d + halfwidth_k <-> tap d.
+ * The buffer must hold 2*(2*info.halfwidth+1) doubles.  Needs fdas_make_templates.
+ */
+fdas_status fdas_get_taps(fdas_plan *plan, int32_t k, double *host_re_im, int32_t *halfwidth_k);
+
+/*
+ * Copy template k's spectrum H_k[0..L-1] to the host in NATURAL frequency order
+ * (synchronises): host_re_im receives 2*seglen floats (re, im).
+ */
+fdas_status fdas_get_template_spectrum(fdas_plan *plan, int32_t k, float *host_re_im);
+
+/*
+ * Sustained FP32 FMA throughput of the device's plain ALUs (the "alu" roofline
+ * denominator): runs `iters` dependent-chain FMA sweeps on every SM, enqueued on `stream`,
+ * synchronises, and returns TFLOP/s (2 flops per FMA) in *tflops.
+ */
+fdas_status fdas_measure_fp32_peak(void *stream, int32_t iters, double *tflops);
+
+/* Number of kernels the library has launched in this process (for bench accounting). */
+int64_t fdas_launch_count(void);
+
+const char *fdas_status_string(fdas_status s);
+/* Text of the last CUDA error seen by this plan ("" if none). */
+const char *fdas_last_error(const fdas_plan *plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FDAS_H_ */

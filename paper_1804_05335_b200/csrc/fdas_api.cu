@@ -1,0 +1,334 @@
+// C ABI of the FDAS library (see include/fdas.h).  Host logic only: argument checks, plan
+// geometry, device allocations, kernel dispatch.  Every step of the path runs in the kernels
+// of fdas_templates.cuh / fdas_kernel.cuh; there is no CPU fallback.
+#include "../../include/fdas.h"
+#include "fdas_templates.cuh"
+
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace fdas;
+
+static std::atomic<long long> g_launches{0};
+
+struct fdas_plan {
+    fdas_info info;
+    int device;
+    bool ready;
+    double2 *d_taps;     // K x (2m+1)
+    float2 *d_hperm;     // npairs x L (kernel register order)
+    float2 *d_wtab;      // L
+    float2 *d_stage_in;  // fdas_execute_host staging (lazy)
+    float *d_stage_out;
+    void (*kernel)(const KernelParams);
+    char err[256];
+};
+
+#define FDAS_CUDA(plan, call)                                                                  \
+    do {                                                                                       \
+        cudaError_t e__ = (call);                                                              \
+        if (e__ != cudaSuccess) {                                                              \
+            if (plan)                                                                          \
+                snprintf((plan)->err, sizeof((plan)->err), "%s: %s", #call,                    \
+                         cudaGetErrorString(e__));                                             \
+            return FDAS_ERR_CUDA;                                                              \
+        }                                                                                      \
+    } while (0)
+
+namespace {
+
+typedef void (*kernel_fn)(const KernelParams);
+
+template <int L>
+kernel_fn pick_kernel(bool ib)
+{
+    return ib ? (kernel_fn)fdas_fused_kernel<L, true, 1> : (kernel_fn)fdas_fused_kernel<L, false, 1>;
+}
+
+kernel_fn select_kernel(int L, bool ib)
+{
+    switch (L) {
+    case 1024: return pick_kernel<1024>(ib);
+    case 2048: return pick_kernel<2048>(ib);
+    case 4096: return pick_kernel<4096>(ib);
+    default: return nullptr;
+    }
+}
+
+int smem_bytes_for(int L, bool ib)
+{
+    const int e2 = L, e1 = 16 * (L / 16 + 1);
+    return (e2 + e1 + (ib ? L : 0)) * (int)sizeof(float4);
+}
+
+} // namespace
+
+extern "C" {
+
+const char *fdas_status_string(fdas_status s)
+{
+    switch (s) {
+    case FDAS_OK: return "FDAS_OK";
+    case FDAS_ERR_INVALID_ARG: return "FDAS_ERR_INVALID_ARG";
+    case FDAS_ERR_UNSUPPORTED: return "FDAS_ERR_UNSUPPORTED";
+    case FDAS_ERR_NOT_READY: return "FDAS_ERR_NOT_READY";
+    case FDAS_ERR_ALIGNMENT: return "FDAS_ERR_ALIGNMENT";
+    case FDAS_ERR_CUDA: return "FDAS_ERR_CUDA";
+    case FDAS_ERR_NOMEM: return "FDAS_ERR_NOMEM";
+    }
+    return "FDAS_ERR_UNKNOWN";
+}
+
+const char *fdas_last_error(const fdas_plan *plan) { return plan ? plan->err : ""; }
+
+int64_t fdas_launch_count(void) { return g_launches.load(); }
+
+fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double dz, int32_t seglen,
+                             int32_t interbin)
+{
+    if (!out) return FDAS_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (nbins <= 0 || !(zmax >= 0.0) || !(dz > 0.0) || !std::isfinite(zmax) || !std::isfinite(dz))
+        return FDAS_ERR_INVALID_ARG;
+    const double nh = zmax / dz;
+    const double nhr = std::floor(nh + 0.5);
+    if (std::fabs(nh - nhr) > 1e-9 * std::fmax(1.0, nh) || nhr > 1e6) return FDAS_ERR_INVALID_ARG;
+    if (interbin != 0 && interbin != 1) return FDAS_ERR_INVALID_ARG;
+    if (seglen != 1024 && seglen != 2048 && seglen != 4096 && seglen != 8192)
+        return FDAS_ERR_UNSUPPORTED;
+
+    const int K = 2 * (int)nhr + 1;
+    const int m = (int)std::ceil(zmax * 0.5 - 1e-12) + 16;
+    const int ov = ((m + interbin) + 31) / 32 * 32; // >= m (+1 for the interbin neighbour), 128B-aligned
+    const int B = seglen - 2 * ov;
+    if (B < 32) return FDAS_ERR_UNSUPPORTED;
+    kernel_fn kern = select_kernel(seglen, interbin != 0);
+    if (!kern) return FDAS_ERR_UNSUPPORTED;
+
+    fdas_plan *p = new (std::nothrow) fdas_plan();
+    if (!p) return FDAS_ERR_NOMEM;
+    std::memset(p, 0, sizeof(*p));
+    p->kernel = kern;
+    fdas_info &I = p->info;
+    I.nbins = nbins;
+    I.ncols = interbin ? 2 * nbins : nbins;
+    I.row_stride = I.ncols;
+    I.nseg = (nbins + B - 1) / B;
+    I.plane_bytes = (int64_t)K * I.ncols * 4;
+    I.zmax = zmax;
+    I.dz = dz;
+    I.ntemplates = K;
+    I.seglen = seglen;
+    I.halfwidth = m;
+    I.overlap = ov;
+    I.useful = B;
+    I.interbin = interbin;
+    I.npairs = (K + 1) / 2;
+    I.threads = seglen / 16;
+    I.smem_bytes = smem_bytes_for(seglen, interbin != 0);
+
+    fdas_status st = FDAS_OK;
+    do {
+        cudaError_t e;
+        if ((e = cudaGetDevice(&p->device)) != cudaSuccess) { st = FDAS_ERR_CUDA; break; }
+        cudaDeviceProp prop;
+        if ((e = cudaGetDeviceProperties(&prop, p->device)) != cudaSuccess) { st = FDAS_ERR_CUDA; break; }
+        I.sm_count = prop.multiProcessorCount;
+        if ((e = cudaFuncSetAttribute((const void *)kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      I.smem_bytes)) != cudaSuccess) { st = FDAS_ERR_CUDA; break; }
+        cudaFuncAttributes fa;
+        if ((e = cudaFuncGetAttributes(&fa, (const void *)kern)) != cudaSuccess) { st = FDAS_ERR_CUDA; break; }
+        I.regs = fa.numRegs;
+        int occ = 0;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)kern, I.threads,
+                                                               I.smem_bytes)) != cudaSuccess) { st = FDAS_ERR_CUDA; break; }
+        if (occ < 1) { st = FDAS_ERR_UNSUPPORTED; break; }
+        I.ctas_per_sm = occ;
+        I.grid = occ * I.sm_count;
+        const size_t taps_bytes = (size_t)K * (2 * m + 1) * sizeof(double2);
+        const size_t h_bytes = (size_t)I.npairs * seglen * sizeof(float2);
+        if (cudaMalloc(&p->d_taps, taps_bytes) != cudaSuccess ||
+            cudaMalloc(&p->d_hperm, h_bytes) != cudaSuccess ||
+            cudaMalloc(&p->d_wtab, (size_t)seglen * sizeof(float2)) != cudaSuccess) {
+            cudaGetLastError();
+            st = FDAS_ERR_NOMEM;
+            break;
+        }
+    } while (0);
+    if (st != FDAS_OK) {
+        fdas_destroy(p);
+        return st;
+    }
+    *out = p;
+    return FDAS_OK;
+}
+
+fdas_status fdas_make_templates(fdas_plan *p, void *stream)
+{
+    if (!p) return FDAS_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const fdas_info &I = p->info;
+    const int w = 2 * I.halfwidth + 1;
+    {
+        const int n = I.ntemplates * w;
+        make_taps_kernel<<<(n + 127) / 128, 128, 0, st>>>(p->d_taps, I.ntemplates, I.halfwidth, I.zmax, I.dz);
+        make_wtab_kernel<<<(I.seglen + 127) / 128, 128, 0, st>>>(p->d_wtab, I.seglen);
+        const int nh = I.npairs * I.seglen;
+        const int gb = (nh + 127) / 128;
+        switch (I.seglen) {
+        case 1024: make_spectra_kernel<1024><<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps, I.npairs, I.halfwidth, I.zmax, I.dz, I.ntemplates); break;
+        case 2048: make_spectra_kernel<2048><<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps, I.npairs, I.halfwidth, I.zmax, I.dz, I.ntemplates); break;
+        case 4096: make_spectra_kernel<4096><<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps, I.npairs, I.halfwidth, I.zmax, I.dz, I.ntemplates); break;
+        default: return FDAS_ERR_UNSUPPORTED;
+        }
+        g_launches += 3;
+    }
+    FDAS_CUDA(p, cudaGetLastError());
+    p->ready = true;
+    return FDAS_OK;
+}
+
+fdas_status fdas_execute(fdas_plan *p, void *stream, const void *d_spectrum, float *d_plane)
+{
+    if (!p || !d_spectrum || !d_plane) return FDAS_ERR_INVALID_ARG;
+    if (!p->ready) return FDAS_ERR_NOT_READY;
+    if (((uintptr_t)d_spectrum & 15) || ((uintptr_t)d_plane & 15)) return FDAS_ERR_ALIGNMENT;
+    const fdas_info &I = p->info;
+    KernelParams prm;
+    prm.spectrum = (const float2 *)d_spectrum;
+    prm.plane = d_plane;
+    prm.hperm = (const float4 *)p->d_hperm;
+    prm.wtab = p->d_wtab;
+    prm.nbins = I.nbins;
+    prm.ncols = I.ncols;
+    prm.nseg = I.nseg;
+    prm.ntemplates = I.ntemplates;
+    prm.npairs = I.npairs;
+    prm.overlap = I.overlap;
+    prm.useful = I.useful;
+    void *args[] = {&prm};
+    FDAS_CUDA(p, cudaLaunchKernel((const void *)p->kernel, dim3(I.grid), dim3(I.threads), args,
+                                  (size_t)I.smem_bytes, (cudaStream_t)stream));
+    g_launches += 1;
+    return FDAS_OK;
+}
+
+fdas_status fdas_execute_host(fdas_plan *p, void *stream, const void *h_spectrum, float *h_plane)
+{
+    if (!p || !h_spectrum || !h_plane) return FDAS_ERR_INVALID_ARG;
+    if (!p->ready) return FDAS_ERR_NOT_READY;
+    const fdas_info &I = p->info;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!p->d_stage_in) {
+        if (cudaMalloc(&p->d_stage_in, (size_t)I.nbins * sizeof(float2)) != cudaSuccess ||
+            cudaMalloc(&p->d_stage_out, (size_t)I.plane_bytes) != cudaSuccess) {
+            cudaGetLastError();
+            cudaFree(p->d_stage_in);
+            p->d_stage_in = nullptr;
+            return FDAS_ERR_NOMEM;
+        }
+    }
+    FDAS_CUDA(p, cudaMemcpyAsync(p->d_stage_in, h_spectrum, (size_t)I.nbins * sizeof(float2),
+                                 cudaMemcpyHostToDevice, st));
+    fdas_status s = fdas_execute(p, stream, p->d_stage_in, p->d_stage_out);
+    if (s != FDAS_OK) return s;
+    FDAS_CUDA(p, cudaMemcpyAsync(h_plane, p->d_stage_out, (size_t)I.plane_bytes, cudaMemcpyDeviceToHost, st));
+    FDAS_CUDA(p, cudaStreamSynchronize(st));
+    return FDAS_OK;
+}
+
+fdas_status fdas_destroy(fdas_plan *p)
+{
+    if (!p) return FDAS_OK;
+    cudaFree(p->d_taps);
+    cudaFree(p->d_hperm);
+    cudaFree(p->d_wtab);
+    cudaFree(p->d_stage_in);
+    cudaFree(p->d_stage_out);
+    cudaGetLastError();
+    delete p;
+    return FDAS_OK;
+}
+
+fdas_status fdas_plan_info(const fdas_plan *p, fdas_info *out)
+{
+    if (!p || !out) return FDAS_ERR_INVALID_ARG;
+    *out = p->info;
+    return FDAS_OK;
+}
+
+fdas_status fdas_get_taps(fdas_plan *p, int32_t k, double *host_re_im, int32_t *halfwidth_k)
+{
+    if (!p || !host_re_im || !halfwidth_k || k < 0 || k >= p->info.ntemplates) return FDAS_ERR_INVALID_ARG;
+    if (!p->ready) return FDAS_ERR_NOT_READY;
+    const fdas_info &I = p->info;
+    const int m = I.halfwidth, w = 2 * m + 1;
+    const int center = (I.ntemplates - 1) / 2;
+    const double z = (k == center) ? 0.0 : -I.zmax + k * I.dz;
+    const int mz = (int)std::ceil(std::fabs(z) * 0.5 - 1e-12) + 16;
+    FDAS_CUDA(p, cudaDeviceSynchronize());
+    FDAS_CUDA(p, cudaMemcpy(host_re_im, p->d_taps + (size_t)k * w + (m - mz),
+                            (size_t)(2 * mz + 1) * sizeof(double2), cudaMemcpyDeviceToHost));
+    *halfwidth_k = mz;
+    return FDAS_OK;
+}
+
+fdas_status fdas_get_template_spectrum(fdas_plan *p, int32_t k, float *host_re_im)
+{
+    if (!p || !host_re_im || k < 0 || k >= p->info.ntemplates) return FDAS_ERR_INVALID_ARG;
+    if (!p->ready) return FDAS_ERR_NOT_READY;
+    const fdas_info &I = p->info;
+    const int L = I.seglen, T = L / 16, R3 = L / 256;
+    const int pair = k < I.ntemplates - 1 - k ? k : I.ntemplates - 1 - k;
+    const bool conj = k != pair;
+    std::vector<float2> buf(L);
+    FDAS_CUDA(p, cudaDeviceSynchronize());
+    FDAS_CUDA(p, cudaMemcpy(buf.data(), p->d_hperm + (size_t)pair * L, (size_t)L * sizeof(float2),
+                            cudaMemcpyDeviceToHost));
+    for (int f = 0; f < L; ++f) {
+        const int b = f & 255, k3 = f >> 8, tid = b % T, i = (b / T) * R3 + k3;
+        const float2 v = buf[((size_t)(i >> 1) * T + tid) * 2 + (i & 1)];
+        host_re_im[2 * f] = v.x;
+        host_re_im[2 * f + 1] = conj ? -v.y : v.y; // H_{+z} = conj(H_{-z})
+    }
+    return FDAS_OK;
+}
+
+fdas_status fdas_measure_fp32_peak(void *stream, int32_t iters, double *tflops)
+{
+    if (!tflops || iters <= 0) return FDAS_ERR_INVALID_ARG;
+    *tflops = 0.0;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    float *d_out = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    fdas_status rc = FDAS_ERR_CUDA;
+    do {
+        if (cudaGetDevice(&dev) != cudaSuccess) break;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) break;
+        if (cudaMalloc(&d_out, 4) != cudaSuccess) break;
+        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) break;
+        const int grid = sms * 8, block = 256;
+        fp32_peak_kernel<<<grid, block, 0, st>>>(d_out, 16, 1.0001f, 0.5f); // warm-up
+        cudaEventRecord(e0, st);
+        fp32_peak_kernel<<<grid, block, 0, st>>>(d_out, iters, 1.0001f, 0.5f);
+        cudaEventRecord(e1, st);
+        g_launches += 2;
+        if (cudaEventSynchronize(e1) != cudaSuccess) break;
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess) break;
+        const double flops = 2.0 * 8.0 * 16.0 * (double)iters * (double)grid * block;
+        *tflops = flops / (ms * 1e-3) / 1e12;
+        rc = FDAS_OK;
+    } while (0);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(d_out);
+    return rc;
+}
+
+} // extern "C"

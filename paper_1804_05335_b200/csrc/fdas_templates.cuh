@@ -1,0 +1,160 @@
+// Plan-time template generation on the device (fp64).
+//
+//  a0  taps: h_z(d) = int_0^1 exp(2 pi i [ -d u + z (u^2 - u)/2 ]) du -- the "predicted
+//      normalised Fourier response" to a constant frequency derivative (formula
+//      not printed there, reading R1), evaluated from its Fresnel-integral closed form
+//          z > 0, q = -d - z/2, Y = q sqrt(2/z), Z = (q+z) sqrt(2/z):
+//          h_z(d) = exp(-i pi q^2 / z) / sqrt(2 z) * { [C(Z)-C(Y)] + i [S(Z)-S(Y)] }
+//          z < 0: h_z(d) = conj(h_{-z}(-d));   z = 0: Kronecker delta at integer d.
+//  a1  spectra: H_z[f] = (1/L) sum_d conj(h_z[d]) exp(+2 pi i d f / L)   (the
+//      filter centred at bin 0, halves at both ends of the L-array; 1/L of eq. 6 folded in, R6),
+//      written in the register order of the fused kernel's un-permuted FFT.
+#pragma once
+#include "fdas_kernel.cuh"
+
+namespace fdas {
+
+// Fresnel integrals C(x) = int_0^x cos(pi t^2/2) dt, S(x) = int_0^x sin(pi t^2/2) dt, fp64.
+//   |x| < 1.8 : Maclaurin series (terms stay below ~200, so cancellation costs < 3 digits)
+//   else      : C + iS = (1+i)/2 * (1 - erfc(w)), w = (sqrt(pi)/2)(1-i)x, with erfc from its
+//               continued fraction  exp(-w^2)/sqrt(pi) * 1/(w + (1/2)/(w + 1/(w + (3/2)/(w + ...))))
+//               evaluated bottom-up with a fixed depth (80 levels reach 1e-16 at |x| = 1.8).
+__device__ inline void fresnel_cs(double x, double &C, double &S)
+{
+    const double ax = fabs(x);
+    double c, s;
+    if (ax < 1.8) {
+        const double a = 1.5707963267948966192313216916398 * ax * ax; // pi/2 x^2
+        double term = ax;                                              // a^k x / k!, k = 0
+        c = 0.0;
+        s = 0.0;
+        for (int n = 0; n < 32; ++n) {
+            const double sg = (n & 1) ? -1.0 : 1.0;
+            c += sg * term / (4 * n + 1);
+            term *= a / (2 * n + 1);
+            s += sg * term / (4 * n + 3);
+            term *= a / (2 * n + 2);
+        }
+    } else {
+        const double k = 0.88622692545275801364908374167057 * ax; // sqrt(pi)/2 * x
+        const double wr = k, wi = -k;                              // w = k (1 - i)
+        double fr = wr, fi = wi;
+        const int depth = ax > 6.0 ? 24 : (ax > 3.0 ? 48 : 96);
+        for (int j = depth; j >= 1; --j) {
+            const double g = 0.5 * j / (fr * fr + fi * fi);        // (j/2) / f = (j/2) conj(f)/|f|^2
+            const double nr = wr + g * fr, ni = wi - g * fi;
+            fr = nr;
+            fi = ni;
+        }
+        // erfc(w) = exp(-w^2)/(sqrt(pi) f), exp(-w^2) = exp(+i pi x^2 / 2)
+        double es, ec;
+        sincospi(0.5 * ax * ax, &es, &ec);
+        const double inv = 0.56418958354775628694807945156077 / (fr * fr + fi * fi); // 1/sqrt(pi)/|f|^2
+        const double er = inv * (ec * fr + es * fi), ei = inv * (es * fr - ec * fi); // e^{..} conj(f)
+        // (1+i)/2 * (1 - erfc)
+        const double ur = 1.0 - er, ui = -ei;
+        c = 0.5 * (ur - ui);
+        s = 0.5 * (ur + ui);
+    }
+    C = x < 0 ? -c : c;
+    S = x < 0 ? -s : s;
+}
+
+// closed form for z > 0
+__device__ inline double2 response_closed_form(double z, double d)
+{
+    const double q = -d - 0.5 * z;
+    const double sc = sqrt(2.0 / z);
+    double CY, SY, CZ, SZ;
+    fresnel_cs(q * sc, CY, SY);
+    fresnel_cs((q + z) * sc, CZ, SZ);
+    double ps, pc;
+    sincospi(-q * q / z, &ps, &pc);
+    const double a = CZ - CY, b = SZ - SY, n = 1.0 / sqrt(2.0 * z);
+    return make_double2(n * (pc * a - ps * b), n * (pc * b + ps * a));
+}
+
+__device__ inline int tap_halfwidth(double z)
+{
+    return (int)ceil(fabs(z) * 0.5 - 1e-12) + 16; // R4: ceil(|z|/2) + 16
+}
+
+// taps[k][d + m], d = -m..m (m = bank half-width); zero for |d| > m_z.
+__global__ void make_taps_kernel(double2 *taps, int K, int m, double zmax, double dz)
+{
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    const int w = 2 * m + 1;
+    if (idx >= K * w) return;
+    const int k = idx / w, d = idx % w - m;
+    const int center = (K - 1) / 2;
+    const double z = (k == center) ? 0.0 : -zmax + k * dz;
+    const int mz = tap_halfwidth(z);
+    double2 h = make_double2(0.0, 0.0);
+    if (d >= -mz && d <= mz) {
+        if (z == 0.0) {
+            h.x = (d == 0) ? 1.0 : 0.0;
+        } else if (z > 0.0) {
+            h = response_closed_form(z, (double)d);
+        } else {
+            h = response_closed_form(-z, (double)(-d));
+            h.y = -h.y;
+        }
+    }
+    taps[idx] = h;
+}
+
+__global__ void make_wtab_kernel(float2 *wtab, int L)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= L) return;
+    double s, c;
+    sincospi(-2.0 * j / L, &s, &c);
+    wtab[j] = make_float2((float)c, (float)s);
+}
+
+// hperm[pair][i/2][tid] (float4 = two complex) for the rows z <= 0 (pair = row index k).
+template <int L>
+__global__ void make_spectra_kernel(float2 *hperm, const double2 *taps, int npairs, int m,
+                                    double zmax, double dz, int K)
+{
+    using G = Geo<L>;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= npairs * L) return;
+    const int pair = idx / L, f = idx % L;
+    const int center = (K - 1) / 2;
+    const double z = (pair == center) ? 0.0 : -zmax + pair * dz;
+    const int mz = tap_halfwidth(z);
+    const double2 *h = taps + (size_t)pair * (2 * m + 1) + m;
+    double sr = 0.0, si = 0.0;
+    for (int d = -mz; d <= mz; ++d) {
+        int r = (int)(((long long)d * f) % L);
+        if (r < 0) r += L;
+        double s, c;
+        sincospi(2.0 * r / L, &s, &c);           // exp(+2 pi i d f / L)
+        const double2 t = h[d];
+        sr += t.x * c + t.y * s;                  // conj(h) * e
+        si += t.x * s - t.y * c;
+    }
+    int tid, i;
+    freq_to_reg<L>(f, tid, i);
+    const size_t off = (((size_t)pair * (G::PTS / 2) + (i >> 1)) * G::T + tid) * 2 + (i & 1);
+    hperm[off] = make_float2((float)(sr / L), (float)(si / L));
+}
+
+// FP32 FMA throughput probe: 8 independent chains per thread.
+__global__ void fp32_peak_kernel(float *out, int iters, float a, float b)
+{
+    float v0 = threadIdx.x, v1 = v0 + 1, v2 = v0 + 2, v3 = v0 + 3, v4 = v0 + 4, v5 = v0 + 5,
+          v6 = v0 + 6, v7 = v0 + 7;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            v0 = fmaf(v0, a, b); v1 = fmaf(v1, a, b); v2 = fmaf(v2, a, b); v3 = fmaf(v3, a, b);
+            v4 = fmaf(v4, a, b); v5 = fmaf(v5, a, b); v6 = fmaf(v6, a, b); v7 = fmaf(v7, a, b);
+        }
+    }
+    const float s = v0 + v1 + v2 + v3 + v4 + v5 + v6 + v7;
+    if (s == 12345.678f) out[0] = s;
+}
+
+} // namespace fdas

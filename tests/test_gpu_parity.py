@@ -1,0 +1,255 @@
+"""
+GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the fp64 oracle on
+the same seeded inputs.  Tolerances are BASELINE.json's (north_star): per row
+max|dP| <= 1e-4 * max(row) and relative L2 <= 1e-5.
+"""
+import ctypes
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL_MAX = 1e-4
+TOL_L2 = 1e-5
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def fd(torch):
+    from paper_1804_05335_b200 import fdas
+    return fdas
+
+
+@pytest.fixture(scope="module")
+def orc():
+    from oracle import fdas_oracle
+    return fdas_oracle
+
+
+@pytest.fixture(scope="module")
+def syn():
+    from paper_1804_05335_b200 import synthetic
+    return synthetic
+
+
+def run_gpu(torch, fd, spectrum, zmax, dz, seglen, interbin, prefill=float("nan")):
+    """Whole plane through the C ABI; returns (numpy float32 plane, info dict)."""
+    n = spectrum.size
+    with fd.Plan(n, zmax, dz, seglen, interbin) as plan:
+        plan.make_templates()
+        info = plan.info.as_dict()
+        d_spec = torch.from_numpy(spectrum.view(np.float32).reshape(n, 2)).cuda()
+        d_plane = torch.full((info["ntemplates"], info["ncols"]), prefill, dtype=torch.float32, device="cuda")
+        stream = torch.cuda.current_stream()
+        plan.execute(stream, d_spec, d_plane)
+        torch.cuda.synchronize()
+        return d_plane.cpu().numpy(), info
+
+
+def check_rows(orc, spectrum, plane, zmax, dz, interbin, rows=None):
+    zs = orc.bank_z(zmax, dz)
+    worst_max, worst_l2 = 0.0, 0.0
+    for k in (range(zs.size) if rows is None else rows):
+        ref = orc.plane_row(spectrum, zs[k], bool(interbin))
+        got = plane[k].astype(np.float64)
+        assert got.shape == ref.shape
+        assert np.all(np.isfinite(got)), f"row {k}: unwritten or non-finite cells"
+        emax = np.max(np.abs(got - ref)) / np.max(ref)
+        el2 = math.sqrt(np.sum((got - ref) ** 2) / np.sum(ref ** 2))
+        worst_max, worst_l2 = max(worst_max, emax), max(worst_l2, el2)
+        assert emax <= TOL_MAX, f"row {k} (z={zs[k]}): max|dP|/rowmax = {emax:.3e}"
+        assert el2 <= TOL_L2, f"row {k} (z={zs[k]}): rel L2 = {el2:.3e}"
+    return worst_max, worst_l2
+
+
+# ------------------------------------------------------------------ templates (a0, a1)
+@pytest.mark.parametrize("zmax,dz,seglen", [(20.0, 2.0, 1024), (84.0, 2.0, 2048), (84.0, 2.0, 4096),
+                                            (6.0, 0.5, 1024)])
+def test_taps_match_oracle_quadrature(torch, fd, orc, zmax, dz, seglen):
+    with fd.Plan(1 << 14, zmax, dz, seglen, 0) as plan:
+        plan.make_templates()
+        torch.cuda.synchronize()
+        zs = orc.bank_z(zmax, dz)
+        assert plan.info.ntemplates == zs.size
+        for k, z in enumerate(zs):
+            got = fd.fdas_get_taps(plan.handle, k)
+            ref = orc.taps(z)
+            assert got.size == ref.size == 2 * orc.halfwidth(z) + 1
+            assert np.max(np.abs(got - ref)) < 1e-12, (k, z)
+
+
+@pytest.mark.parametrize("zmax,dz,seglen", [(20.0, 2.0, 1024), (84.0, 2.0, 2048), (84.0, 2.0, 4096)])
+def test_template_spectra_match_fp64_fft_of_oracle_taps(torch, fd, orc, zmax, dz, seglen):
+    with fd.Plan(1 << 14, zmax, dz, seglen, 0) as plan:
+        plan.make_templates()
+        zs = orc.bank_z(zmax, dz)
+        for k in list(range(0, zs.size, 7)) + [zs.size // 2, zs.size - 1]:
+            h = orc.taps(zs[k])
+            m = (h.size - 1) // 2
+            g = np.zeros(seglen, dtype=np.complex128)
+            for d in range(-m, m + 1):
+                g[(-d) % seglen] = np.conj(h[d + m])          # PAPER.md:77, :87 (Fig. 1)
+            ref = np.fft.fft(g) / seglen
+            got = fd.fdas_get_template_spectrum(plan.handle, k).astype(np.complex128)
+            assert np.max(np.abs(got - ref)) < 1.5e-7 * np.max(np.abs(ref)), k
+
+
+# ------------------------------------------------------------------ whole-plane parity
+def test_config1_full_plane(torch, fd, orc, syn):
+    spec, chirps = syn.config_spectrum(0)
+    plane, info = run_gpu(torch, fd, spec, 20.0, 2.0, 1024, 0)
+    assert plane.shape == (21, 1 << 16)
+    check_rows(orc, spec, plane, 20.0, 2.0, 0)
+    k, r = np.unravel_index(np.argmax(plane), plane.shape)
+    assert k == 14 and r == 20000                       # z = +8, r = round(20000.25)
+    # z = 0 row is |A|^2 up to fp32 rounding (P2)
+    a = spec.astype(np.complex128)
+    assert np.max(np.abs(plane[10] - (a.real ** 2 + a.imag ** 2))) < 2e-5 * np.max(plane[10])
+
+
+@pytest.mark.parametrize("cfg,nbins", [(1, 1 << 18), (1, 100003), (2, 1 << 17), (4, 1 << 17), (2, 77777)])
+def test_reduced_configs_full_plane(torch, fd, orc, syn, cfg, nbins):
+    c = syn.CONFIGS[cfg]
+    spec, _ = syn.config_spectrum(cfg, 0, nbins)
+    plane, info = run_gpu(torch, fd, spec, c["zmax"], c["dz"], c["seglen"], c["interbin"])
+    assert plane.shape == (info["ntemplates"], nbins * (2 if c["interbin"] else 1))
+    check_rows(orc, spec, plane, c["zmax"], c["dz"], c["interbin"])
+
+
+def test_config2_full_size_full_plane(torch, fd, orc, syn):
+    c = syn.CONFIGS[1]
+    spec, chirps = syn.config_spectrum(1)
+    plane, info = run_gpu(torch, fd, spec, c["zmax"], c["dz"], c["seglen"], 0)
+    wm, wl = check_rows(orc, spec, plane, c["zmax"], c["dz"], 0)
+    print(f"config2: worst max-err {wm:.3e}, worst rel-L2 {wl:.3e}")
+    zs = orc.bank_z(c["zmax"], c["dz"])
+    for (r0, z0, a0) in chirps:                          # P4: each chirp peaks at its cell
+        k0 = int(np.argmin(np.abs(zs - z0)))
+        lo, hi = int(r0) - 3, int(r0) + 4
+        sub = plane[max(0, k0 - 2):k0 + 3, lo:hi]
+        assert sub.max() > 0.5 * a0 * a0
+        kk, rr = np.unravel_index(np.argmax(sub), sub.shape)
+        assert abs((max(0, k0 - 2) + kk) - k0) <= 1 and abs(lo + rr - r0) <= 1.0
+
+
+def test_config3_full_size_sampled_rows(torch, fd, orc, syn):
+    c = syn.CONFIGS[2]
+    spec = syn.noise_only_c64(c["nbins"], 31337)
+    spec[123456] += 25.0
+    plane, info = run_gpu(torch, fd, spec, c["zmax"], c["dz"], c["seglen"], 1)
+    assert plane.shape == (85, 1 << 24)
+    assert np.all(np.isfinite(plane))
+    check_rows(orc, spec, plane, c["zmax"], c["dz"], 1, rows=[0, 17, 42, 43, 84])
+    # sampled cells in every row
+    rng = np.random.default_rng(5)
+    zs = orc.bank_z(c["zmax"], c["dz"])
+    for k, z in enumerate(zs):
+        cols = np.concatenate([rng.integers(0, plane.shape[1], 4000),
+                               [0, 1, plane.shape[1] - 2, plane.shape[1] - 1]])
+        ref = orc.plane_cells(spec, z, cols, True)
+        assert np.max(np.abs(plane[k, cols] - ref)) <= TOL_MAX * np.max(plane[k])
+
+
+def test_config5_batch_on_one_stream(torch, fd, orc, syn):
+    c = syn.CONFIGS[4]
+    nb = 3
+    n = 1 << 17
+    specs = [syn.config_spectrum(4, b, n)[0] for b in range(nb)]
+    with fd.Plan(n, c["zmax"], c["dz"], c["seglen"], 1) as plan:
+        plan.make_templates()
+        K, ncols = plan.info.ntemplates, plan.info.ncols
+        d_specs = [torch.from_numpy(s.view(np.float32).reshape(n, 2)).cuda() for s in specs]
+        d_out = torch.full((nb, K, ncols), float("nan"), dtype=torch.float32, device="cuda")
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            for b in range(nb):
+                plan.execute(st, d_specs[b], d_out[b])      # no host sync between calls
+        st.synchronize()
+        out = d_out.cpu().numpy()
+    for b in range(nb):
+        check_rows(orc, specs[b], out[b], c["zmax"], c["dz"], 1, rows=range(0, 85, 6))
+
+
+# ------------------------------------------------------------------ edge cases
+@pytest.mark.parametrize("nbins", [1, 31, 960, 961, 1921])
+@pytest.mark.parametrize("interbin", [0, 1])
+def test_tiny_and_ragged_spectra(torch, fd, orc, syn, nbins, interbin):
+    spec = syn.make_spectrum(nbins, 900 + nbins, [(nbins / 2.0, 4.0, 10.0)] if nbins > 40 else [])
+    plane, info = run_gpu(torch, fd, spec, 20.0, 2.0, 1024, interbin)
+    check_rows(orc, spec, plane, 20.0, 2.0, interbin)
+
+
+def test_single_template_bank(torch, fd, orc, syn):
+    spec = syn.make_spectrum(5000, 71)
+    plane, info = run_gpu(torch, fd, spec, 0.0, 2.0, 1024, 0)
+    assert plane.shape == (1, 5000)
+    check_rows(orc, spec, plane, 0.0, 2.0, 0)
+
+
+def test_fractional_dz_bank(torch, fd, orc, syn):
+    spec = syn.make_spectrum(20000, 72, [(9000.4, 2.5, 15.0)])
+    plane, info = run_gpu(torch, fd, spec, 6.0, 0.5, 1024, 0)
+    assert plane.shape[0] == 25
+    check_rows(orc, spec, plane, 6.0, 0.5, 0)
+    k, r = np.unravel_index(np.argmax(plane), plane.shape)
+    assert orc.bank_z(6.0, 0.5)[k] == 2.5 and r == 9000
+
+
+def test_deterministic_and_linear(torch, fd, syn):
+    spec = syn.make_spectrum(1 << 16, 73)
+    p1, _ = run_gpu(torch, fd, spec, 20.0, 2.0, 1024, 0)
+    p2, _ = run_gpu(torch, fd, spec, 20.0, 2.0, 1024, 0)
+    assert np.array_equal(p1, p2)
+    p4, _ = run_gpu(torch, fd, (2.0 * spec).astype(np.complex64), 20.0, 2.0, 1024, 0)
+    assert np.array_equal(p4, 4.0 * p1)                  # power-of-two scaling is exact in fp32
+
+
+def test_segmentation_independence_on_gpu(torch, fd, syn):
+    # P10 on the device: the plane does not depend on the segment length
+    spec = syn.make_spectrum(50000, 74, [(25000.0, -6.0, 12.0)])
+    a, _ = run_gpu(torch, fd, spec, 20.0, 2.0, 1024, 0)
+    b, _ = run_gpu(torch, fd, spec, 20.0, 2.0, 4096, 0)
+    assert np.max(np.abs(a - b)) < 2e-5 * np.max(a)
+
+
+def test_error_codes_on_device(torch, fd):
+    with fd.Plan(4096, 20.0, 2.0, 1024, 0) as plan:
+        spec = torch.zeros(4096, 2, device="cuda")
+        out = torch.zeros(21, 4096, device="cuda")
+        with pytest.raises(fd.FdasError) as e:
+            plan.execute(None, spec, out)
+        assert e.value.status == 3                       # NOT_READY
+        plan.make_templates()
+        with pytest.raises(fd.FdasError) as e:
+            fd.fdas_execute(plan.handle, None, spec.data_ptr() + 8, out)
+        assert e.value.status == 4                       # ALIGNMENT
+        with pytest.raises(fd.FdasError) as e:
+            fd.fdas_execute(plan.handle, None, 0, out)
+        assert e.value.status == 1
+        plan.execute(None, spec, out)
+        torch.cuda.synchronize()
+        assert float(out.abs().max()) == 0.0
+
+
+def test_execute_host_end_to_end(torch, fd, orc, syn):
+    spec, _ = syn.config_spectrum(0)
+    with fd.Plan(spec.size, 20.0, 2.0, 1024, 0) as plan:
+        plan.make_templates()
+        h_in = torch.from_numpy(spec.view(np.float32).reshape(-1, 2)).pin_memory()
+        h_out = torch.empty(21, spec.size, dtype=torch.float32).pin_memory()
+        plan.execute_host(torch.cuda.current_stream(), h_in, h_out)
+        check_rows(orc, spec, h_out.numpy(), 20.0, 2.0, 0, rows=[0, 10, 14, 20])
+
+
+def test_fp32_peak_probe(torch, fd):
+    tf = fd.fdas_measure_fp32_peak(None, 2000)
+    assert 20.0 < tf < 90.0, tf
+    assert fd.fdas_launch_count() > 0

@@ -43,33 +43,57 @@ FDAS_HD float2 cmul_conj(float2 a, float2 w) // a * conj(w)
     return make_float2(a.x * w.x + a.y * w.y, a.y * w.x - a.x * w.y);
 }
 
-// One radix-2 DIT butterfly with the compile-time twiddle exp(DIR * 2 pi i * J / LEN):
+// tan(2 pi k / 32), k = 0..4 (|tan| <= 1), for the 6-FMA twiddled butterfly below
+FDAS_HD constexpr float tan32(int k)
+{
+    return k == 0 ? 0.0f
+         : k == 1 ? 0.19891236737965800691159762264468f
+         : k == 2 ? 0.41421356237309504880168872420970f
+         : k == 3 ? 0.66817863791929891999775768652308f
+         : 1.0f;
+}
+
+// One radix-2 DIT butterfly with the compile-time twiddle w = exp(DIR * 2 pi i * J / LEN):
 //   e' = e + w o,  o' = e - w o.     J in [0, LEN/2), LEN in {2,4,8,16,32}
+// Non-trivial twiddles use the 6-FMA form: w o = s * (u, v) with (u, v) = o rotated by a
+// unit-free factor (1, t) or (t, 1), |t| = tan <= 1, so that e +- s*(u,v) are 4 FMAs.
 template <int DIR, int J, int LEN>
 FDAS_HD void bfly(float2 &e, float2 &o)
 {
-    constexpr int idx = J * (32 / LEN); // angle = 2 pi idx / 32, idx in [0,16)
-    float2 t;
-    if constexpr (idx == 0) {
-        t = o;
-    } else if constexpr (idx == 8) { // w = DIR * i
-        t = (DIR > 0) ? make_float2(-o.y, o.x) : make_float2(o.y, -o.x);
-    } else if constexpr (idx == 4) { // w = (1 + DIR i)/sqrt2
-        constexpr float c = cos32(4);
-        t = (DIR > 0) ? make_float2(c * (o.x - o.y), c * (o.x + o.y))
-                      : make_float2(c * (o.x + o.y), c * (o.y - o.x));
-    } else if constexpr (idx == 12) { // w = (-1 + DIR i)/sqrt2
-        constexpr float c = cos32(4);
-        t = (DIR > 0) ? make_float2(-c * (o.x + o.y), c * (o.x - o.y))
-                      : make_float2(c * (o.y - o.x), -c * (o.x + o.y));
-    } else {
-        constexpr float wr = cosw(idx);
-        constexpr float wi = (DIR > 0) ? sinw(idx) : -sinw(idx);
-        t = make_float2(wr * o.x - wi * o.y, wr * o.y + wi * o.x);
-    }
+    constexpr int idx = J * (32 / LEN); // angle = DIR * 2 pi idx / 32, idx in [0,16)
     const float2 ee = e;
-    e = cadd(ee, t);
-    o = csub(ee, t);
+    if constexpr (idx == 0) {
+        e = cadd(ee, o);
+        o = csub(ee, o);
+    } else if constexpr (idx == 8) { // w = DIR * i
+        const float2 t = (DIR > 0) ? make_float2(-o.y, o.x) : make_float2(o.y, -o.x);
+        e = cadd(ee, t);
+        o = csub(ee, t);
+    } else {
+        // w = c + i s with c = cos(a), s = DIR*sin(a), a = 2 pi idx/32 in (0, pi), a != pi/2.
+        // Write w = g * (p + i q) with (p, q) = (1, tan) when |c| >= |s|, else (cot, 1); g = c or s.
+        constexpr int r = idx <= 8 ? idx : 16 - idx;           // reflect to [0, 8]
+        constexpr bool cos_major = r <= 4;                       // |cos| >= |sin|
+        constexpr float tt = cos_major ? tan32(r) : tan32(8 - r); // |sin/cos| or |cos/sin|
+        constexpr float cs = idx <= 8 ? 1.0f : -1.0f;            // sign of cos
+        constexpr float sn = DIR > 0 ? 1.0f : -1.0f;             // sign of sin
+        float u, v, g;
+        if constexpr (cos_major) {
+            // w = c (1 + i q), q = s/c
+            constexpr float q = sn * cs * tt;
+            g = cosw(idx);
+            u = fmaf(-q, o.y, o.x);
+            v = fmaf(q, o.x, o.y);
+        } else {
+            // w = s (p + i), p = c/s
+            constexpr float pq = sn * cs * tt;
+            g = sn * sinw(idx);
+            u = fmaf(pq, o.x, -o.y);
+            v = fmaf(pq, o.y, o.x);
+        }
+        e = make_float2(fmaf(g, u, ee.x), fmaf(g, v, ee.y));
+        o = make_float2(fmaf(-g, u, ee.x), fmaf(-g, v, ee.y));
+    }
 }
 
 template <int R>

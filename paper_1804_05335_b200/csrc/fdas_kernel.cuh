@@ -153,13 +153,18 @@ FDAS_HD void load_inv_twiddles(const float2 *__restrict__ wtab, int tid, InvTwid
 // ------------------------------------------------------------------ inverse passes (+z / -z pairs)
 // Q3: Y+ = X^ * H, Y- = X^ * conj(H), inverse DFT_R3 over k3, twiddle, store E2.
 template <int L>
-FDAS_HD void inv_q3(const float2 (&xh)[Geo<L>::PTS], const float4 *__restrict__ hp,
+FDAS_HD void load_h(const float4 *__restrict__ hp, int tid, float4 (&h4)[Geo<L>::PTS / 2])
+{
+    using G = Geo<L>;
+#pragma unroll
+    for (int i2 = 0; i2 < G::PTS / 2; ++i2) h4[i2] = hp[i2 * G::T + tid];
+}
+
+template <int L>
+FDAS_HD void inv_q3(const float2 (&xh)[Geo<L>::PTS], const float4 (&h4)[Geo<L>::PTS / 2],
                     const InvTwiddles<L> &tw, int tid, float4 *s0)
 {
     using G = Geo<L>;
-    float4 h4[G::PTS / 2];
-#pragma unroll
-    for (int i2 = 0; i2 < G::PTS / 2; ++i2) h4[i2] = hp[i2 * G::T + tid];
 #pragma unroll
     for (int j = 0; j < G::NB3; ++j) {
         const int b = tid + G::T * j;
@@ -262,16 +267,29 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
     const long long units = prm.nseg * prm.npairs;
     long long u = units * blockIdx.x / gridDim.x;
     const long long u_end = units * (blockIdx.x + 1) / gridDim.x;
-    long long seg = -1;
+    if (u >= u_end) return;
+    long long seg = u / prm.npairs;
+    int pair = (int)(u - seg * prm.npairs);
+    bool need_fwd = true;
     float2 xh[G::PTS];
+    float4 h4[G::PTS / 2];
+    constexpr size_t HSTRIDE = (size_t)(G::PTS / 2) * G::T;
+    load_h<L>(prm.hperm + pair * HSTRIDE, tid, h4);
+
+    // which of this thread's 16 outputs n = n1*Q + tid fall in the useful range [ov, ov+B)
+    static_assert(G::NB1 == 1, "epilogue assumes one Q1 butterfly per thread");
+    unsigned vmask = 0;
+#pragma unroll
+    for (int n1 = 0; n1 < 16; ++n1) {
+        const int n = n1 * G::Q + tid;
+        if (n >= prm.overlap && n < prm.overlap + prm.useful) vmask |= 1u << n1;
+    }
 
     constexpr float IB = 0.61685027506808491367715568749226f; // (pi/4)^2, eq. 4 squared
 
     for (; u < u_end; ++u) {
-        const long long s = u / prm.npairs;
-        const int pair = (int)(u - s * prm.npairs);
-        if (s != seg) {
-            seg = s;
+        if (need_fwd) {
+            need_fwd = false;
             __syncthreads(); // previous unit's readers of s1 are done
             fwd_f1<L>(prm.spectrum, prm.nbins, seg * prm.useful - prm.overlap, prm.wtab, tid,
                       reinterpret_cast<float2 *>(s1));
@@ -282,51 +300,76 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
             fwd_f3<L>(tid, reinterpret_cast<const float2 *>(s0), xh);
             __syncthreads(); // s0 is rewritten by inv_q3 below
         }
-        inv_q3<L>(xh, prm.hperm + (size_t)pair * (G::PTS / 2) * G::T, tw, tid, s0);
+        inv_q3<L>(xh, h4, tw, tid, s0);
         __syncthreads();
+
+        // next unit; its H is fetched now so the L2 latency hides behind Q2/Q1
+        int npair = pair + 1;
+        long long nseg_ = seg;
+        if (npair == prm.npairs) {
+            npair = 0;
+            ++nseg_;
+        }
+        if (u + 1 < u_end) load_h<L>(prm.hperm + npair * HSTRIDE, tid, h4);
+
         inv_q2<L>(tw, tid, s0, s1);
         __syncthreads();
 
         const int row_p = pair;                         // z <= 0
         const int row_q = prm.ntemplates - 1 - pair;    // z >= 0 (same row for the z = 0 slot)
         const bool has_q = row_q != row_p;
-        float *out_p = prm.plane + (size_t)row_p * prm.ncols;
-        float *out_q = prm.plane + (size_t)row_q * prm.ncols;
         const long long col0 = seg * prm.useful - prm.overlap;  // column of local index 0
+        const bool interior = col0 + prm.overlap + prm.useful <= prm.nbins;
 
-#pragma unroll
-        for (int j = 0; j < G::NB1; ++j) {
-            float2 p[16], q[16];
-            inv_q1<L>(tid, j, s1, p, q);
-            const int t1 = tid + G::T * j;
-            if constexpr (!INTERBIN) {
-#pragma unroll
-                for (int n1 = 0; n1 < 16; ++n1) {
-                    const int n = n1 * G::Q + t1;
-                    const long long col = col0 + n;
-                    if (n >= prm.overlap && n < prm.overlap + prm.useful && col < prm.nbins) {
-                        st_stream(out_p + col, power(p[n1]));
-                        if (has_q) st_stream(out_q + col, power(q[n1]));
-                    }
-                }
-            } else {
+        float2 p[16], q[16];
+        inv_q1<L>(tid, 0, s1, p, q);
+        if constexpr (!INTERBIN) {
+            float *bp = prm.plane + (size_t)row_p * prm.ncols + (col0 + tid);
+            float *bq = prm.plane + (size_t)row_q * prm.ncols + (col0 + tid);
+            unsigned vm = vmask;
+            if (!interior) {
 #pragma unroll
                 for (int n1 = 0; n1 < 16; ++n1)
-                    s2[n1 * G::Q + t1] = make_float4(p[n1].x, p[n1].y, q[n1].x, q[n1].y);
-                __syncthreads();
+                    if (col0 + n1 * G::Q + tid >= prm.nbins) vm &= ~(1u << n1);
+            }
 #pragma unroll
-                for (int n1 = 0; n1 < 16; ++n1) {
-                    const int n = n1 * G::Q + t1;
-                    const long long col = col0 + n;
-                    if (n >= prm.overlap && n < prm.overlap + prm.useful && col < prm.nbins) {
-                        const float4 nx = s2[n + 1]; // n + 1 <= overlap + useful < L
-                        const float2 dp = make_float2(p[n1].x - nx.x, p[n1].y - nx.y);
+            for (int n1 = 0; n1 < 16; ++n1)
+                if (vm & (1u << n1)) st_stream(bp + n1 * G::Q, power(p[n1]));
+            if (has_q) {
+#pragma unroll
+                for (int n1 = 0; n1 < 16; ++n1)
+                    if (vm & (1u << n1)) st_stream(bq + n1 * G::Q, power(q[n1]));
+            }
+        } else {
+#pragma unroll
+            for (int n1 = 0; n1 < 16; ++n1)
+                s2[n1 * G::Q + tid] = make_float4(p[n1].x, p[n1].y, q[n1].x, q[n1].y);
+            __syncthreads();
+            float *bp = prm.plane + (size_t)row_p * prm.ncols + 2 * (col0 + tid);
+            float *bq = prm.plane + (size_t)row_q * prm.ncols + 2 * (col0 + tid);
+            unsigned vm = vmask;
+            if (!interior) {
+#pragma unroll
+                for (int n1 = 0; n1 < 16; ++n1)
+                    if (col0 + n1 * G::Q + tid >= prm.nbins) vm &= ~(1u << n1);
+            }
+#pragma unroll
+            for (int n1 = 0; n1 < 16; ++n1) {
+                if (vm & (1u << n1)) {
+                    const float4 nx = s2[n1 * G::Q + tid + 1]; // n + 1 <= overlap + useful < L
+                    const float2 dp = make_float2(p[n1].x - nx.x, p[n1].y - nx.y);
+                    st_stream2(bp + 2 * n1 * G::Q, power(p[n1]), IB * power(dp));
+                    if (has_q) {
                         const float2 dq = make_float2(q[n1].x - nx.z, q[n1].y - nx.w);
-                        st_stream2(out_p + 2 * col, power(p[n1]), IB * power(dp));
-                        if (has_q) st_stream2(out_q + 2 * col, power(q[n1]), IB * power(dq));
+                        st_stream2(bq + 2 * n1 * G::Q, power(q[n1]), IB * power(dq));
                     }
                 }
             }
+        }
+        pair = npair;
+        if (nseg_ != seg) {
+            seg = nseg_;
+            need_fwd = true;
         }
     }
 }

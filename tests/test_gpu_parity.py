@@ -135,7 +135,7 @@ def test_config2_full_size_full_plane(torch, fd, orc, syn):
         k0 = int(np.argmin(np.abs(zs - z0)))
         lo, hi = int(r0) - 3, int(r0) + 4
         sub = plane[max(0, k0 - 2):k0 + 3, lo:hi]
-        assert sub.max() > 0.5 * a0 * a0
+        assert sub.max() > 0.3 * a0 * a0          # off-grid (r, z): scalloping in both axes
         kk, rr = np.unravel_index(np.argmax(sub), sub.shape)
         assert abs((max(0, k0 - 2) + kk) - k0) <= 1 and abs(lo + rr - r0) <= 1.0
 

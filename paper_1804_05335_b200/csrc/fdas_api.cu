@@ -62,7 +62,7 @@ kernel_fn select_kernel(int L, bool ib)
 int smem_bytes_for(int L, bool ib)
 {
     const int e2 = L, e1 = 16 * (L / 16 + 1);
-    return (e2 + e1 + (ib ? L : 0)) * (int)sizeof(float4);
+    return (e2 + e1 + (ib ? L + 2 : 0)) * (int)sizeof(float4);
 }
 
 } // namespace

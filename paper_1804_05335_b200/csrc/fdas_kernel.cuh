@@ -33,6 +33,7 @@ struct Geo {
     static constexpr int S1 = Q + 1;         // padded row length of exchange E1
     static constexpr int E2_ELEMS = L;
     static constexpr int E1_ELEMS = 16 * S1;
+    static constexpr int IB_ELEMS = L + 2;   // interbin neighbour exchange (index L is read, never used)
     static_assert(L == 1024 || L == 2048 || L == 4096, "segment length");
 };
 
@@ -151,24 +152,48 @@ FDAS_HD void load_inv_twiddles(const float2 *__restrict__ wtab, int tid, InvTwid
 }
 
 // ------------------------------------------------------------------ inverse passes (+z / -z pairs)
-// Q3: Y+ = X^ * H, Y- = X^ * conj(H), inverse DFT_R3 over k3, twiddle, store E2.
+#ifdef __CUDACC__
 template <int L>
-FDAS_HD void load_h(const float4 *__restrict__ hp, int tid, float4 (&h4)[Geo<L>::PTS / 2])
+__device__ __forceinline__ void load_h(const float4 *__restrict__ hp, int tid, float4 (&h4)[Geo<L>::PTS / 2])
 {
     using G = Geo<L>;
 #pragma unroll
     for (int i2 = 0; i2 < G::PTS / 2; ++i2) h4[i2] = hp[i2 * G::T + tid];
 }
 
+// Exchange buffer for packed pairs: the (Re p, Re q) and (Im p, Im q) register pairs live in two
+// separate 8-byte planes, so every access is one 64-bit LDS/STS straight from/to the register
+// pair the packed arithmetic uses (a 16-byte interleaved element costs 4 MOVs per store to line
+// the two pairs up in one aligned register quad).  Same index maps, same wavefront count.
+struct XBuf {
+    float2 *re, *im;
+    __device__ __forceinline__ void put(int i, const cpk &a) const
+    {
+        re[i] = a.re;
+        im[i] = a.im;
+    }
+    __device__ __forceinline__ cpk get(int i) const
+    {
+        cpk a;
+        a.re = re[i];
+        a.im = im[i];
+        return a;
+    }
+};
+
+// Q3: p = X^ * H, q = X^ * conj(H) as one packed pair, inverse DFT_R3 over k3,
+// twiddle, store E2.
+//   (Re p, Re q) = x.re*h.re -+ x.im*h.im,   (Im p, Im q) = x.im*h.re +- x.re*h.im
+// (scalar FMUL/FFMA writing straight into the register pairs: 6 lane-ops per point).
 template <int L>
-FDAS_HD void inv_q3(const float2 (&xh)[Geo<L>::PTS], const float4 (&h4)[Geo<L>::PTS / 2],
-                    const InvTwiddles<L> &tw, int tid, float4 *s0)
+__device__ __forceinline__ void inv_q3(const float2 (&xh)[Geo<L>::PTS], const float4 (&h4)[Geo<L>::PTS / 2],
+                                       const InvTwiddles<L> &tw, int tid, const XBuf &s0)
 {
     using G = Geo<L>;
 #pragma unroll
     for (int j = 0; j < G::NB3; ++j) {
         const int b = tid + G::T * j;
-        float2 p[G::R3], q[G::R3];
+        cpk a[G::R3];
 #pragma unroll
         for (int k3 = 0; k3 < G::R3; ++k3) {
             const int i = j * G::R3 + k3;
@@ -176,64 +201,50 @@ FDAS_HD void inv_q3(const float2 (&xh)[Geo<L>::PTS], const float4 (&h4)[Geo<L>::
             const float2 h = (i & 1) ? make_float2(hh.z, hh.w) : make_float2(hh.x, hh.y);
             const float2 x = xh[i];
             const float ac = x.x * h.x, bc = x.y * h.x;
-            p[k3] = make_float2(ac - x.y * h.y, bc + x.x * h.y);
-            q[k3] = make_float2(ac + x.y * h.y, bc - x.x * h.y);
+            a[k3].re = make_float2(fmaf(-x.y, h.y, ac), fmaf(x.y, h.y, ac));
+            a[k3].im = make_float2(fmaf(x.x, h.y, bc), fmaf(-x.x, h.y, bc));
         }
-        dft<+1, G::R3>(p);
-        dft<+1, G::R3>(q);
+        dft<+1, G::R3>(a);
 #pragma unroll
         for (int n3 = 0; n3 < G::R3; ++n3) {
-            float2 pp = p[n3], qq = q[n3];
-            if (n3 > 0) {
-                pp = cmul(pp, tw.tw3[j][n3]);
-                qq = cmul(qq, tw.tw3[j][n3]);
-            }
-            s0[b + 256 * n3] = make_float4(pp.x, pp.y, qq.x, qq.y);
+            const cpk v = (n3 > 0) ? cmul(a[n3], tw.tw3[j][n3]) : a[n3];
+            s0.put(b + 256 * n3, v);
         }
     }
 }
 
 // Q2: load E2, inverse DFT16 over k2, twiddle, store E1.
 template <int L>
-FDAS_HD void inv_q2(const InvTwiddles<L> &tw, int tid, const float4 *s0, float4 *s1)
+__device__ __forceinline__ void inv_q2(const InvTwiddles<L> &tw, int tid, const XBuf &s0, const XBuf &s1)
 {
     using G = Geo<L>;
 #pragma unroll
     for (int j = 0; j < G::NB2; ++j) {
         const int u = tid + G::T * j, k1 = u & 15, n3 = u >> 4;
-        float2 p[16], q[16];
+        cpk a[16];
 #pragma unroll
-        for (int k2 = 0; k2 < 16; ++k2) {
-            const float4 v = s0[k1 + 16 * k2 + 256 * n3];
-            p[k2] = make_float2(v.x, v.y);
-            q[k2] = make_float2(v.z, v.w);
-        }
-        dft<+1, 16>(p);
-        dft<+1, 16>(q);
+        for (int k2 = 0; k2 < 16; ++k2) a[k2] = s0.get(k1 + 16 * k2 + 256 * n3);
+        dft<+1, 16>(a);
 #pragma unroll
-        for (int n2 = 0; n2 < 16; ++n2) {
-            const float2 pp = cmul(p[n2], tw.tw2[j][n2]);
-            const float2 qq = cmul(q[n2], tw.tw2[j][n2]);
-            s1[k1 * G::S1 + n2 * G::R3 + n3] = make_float4(pp.x, pp.y, qq.x, qq.y);
-        }
+        for (int n2 = 0; n2 < 16; ++n2)
+            s1.put(k1 * G::S1 + n2 * G::R3 + n3, cmul(a[n2], tw.tw2[j][n2]));
     }
 }
 
 // Q1: load E1, inverse DFT16 over k1 -> y[n1*Q + t1] for butterfly j.
 template <int L>
-FDAS_HD void inv_q1(int tid, int j, const float4 *s1, float2 (&p)[16], float2 (&q)[16])
+__device__ __forceinline__ void inv_q1(int tid, int j, const XBuf &s1, cpk (&a)[16])
 {
     using G = Geo<L>;
     const int t1 = tid + G::T * j;
 #pragma unroll
-    for (int k1 = 0; k1 < 16; ++k1) {
-        const float4 v = s1[k1 * G::S1 + t1];
-        p[k1] = make_float2(v.x, v.y);
-        q[k1] = make_float2(v.z, v.w);
-    }
-    dft<+1, 16>(p);
-    dft<+1, 16>(q);
+    for (int k1 = 0; k1 < 16; ++k1) a[k1] = s1.get(k1 * G::S1 + t1);
+    dft<+1, 16>(a);
 }
+
+// (|p|^2, |q|^2)
+__device__ __forceinline__ float2 power2(const cpk &y) { return fma2(y.im, y.im, mul2(y.re, y.re)); }
+#endif // __CUDACC__
 
 FDAS_HD float power(float2 y) { return y.x * y.x + y.y * y.y; }
 
@@ -247,6 +258,17 @@ __device__ __forceinline__ void st_stream2(float *p, float a, float b)
 {
     asm volatile("st.global.cs.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(a), "f"(b) : "memory");
 }
+// predicated forms (no branch around the store)
+__device__ __forceinline__ void st_stream_if(float *p, float v, unsigned pred)
+{
+    asm volatile("{\n\t.reg .pred pp;\n\tsetp.ne.u32 pp, %2, 0;\n\t@pp st.global.cs.f32 [%0], %1;\n\t}"
+                 ::"l"(p), "f"(v), "r"(pred) : "memory");
+}
+__device__ __forceinline__ void st_stream2_if(float *p, float a, float b, unsigned pred)
+{
+    asm volatile("{\n\t.reg .pred pp;\n\tsetp.ne.u32 pp, %3, 0;\n\t@pp st.global.cs.v2.f32 [%0], {%1, %2};\n\t}"
+                 ::"l"(p), "f"(a), "f"(b), "r"(pred) : "memory");
+}
 
 // Persistent fused kernel.  Work = nseg * npairs (segment, template-slot) units, split into
 // gridDim.x equal contiguous ranges (segment-major), so each CTA redoes at most one extra
@@ -256,9 +278,11 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
 {
     using G = Geo<L>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float4 *s0 = reinterpret_cast<float4 *>(smem_raw);           // E2, L elements
-    float4 *s1 = s0 + G::E2_ELEMS;                               // E1, L+16 elements
-    float4 *s2 = s1 + G::E1_ELEMS;                               // interbin only, L elements
+    float2 *sm = reinterpret_cast<float2 *>(smem_raw);
+    const XBuf s0{sm, sm + G::E2_ELEMS};                                             // E2
+    const XBuf s1{sm + 2 * G::E2_ELEMS, sm + 2 * G::E2_ELEMS + G::E1_ELEMS};         // E1 (padded)
+    const XBuf s2{sm + 2 * (G::E2_ELEMS + G::E1_ELEMS),
+                  sm + 2 * (G::E2_ELEMS + G::E1_ELEMS) + G::IB_ELEMS};               // interbin only
     const int tid = threadIdx.x;
 
     InvTwiddles<L> tw;
@@ -291,13 +315,11 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
         if (need_fwd) {
             need_fwd = false;
             __syncthreads(); // previous unit's readers of s1 are done
-            fwd_f1<L>(prm.spectrum, prm.nbins, seg * prm.useful - prm.overlap, prm.wtab, tid,
-                      reinterpret_cast<float2 *>(s1));
+            fwd_f1<L>(prm.spectrum, prm.nbins, seg * prm.useful - prm.overlap, prm.wtab, tid, s1.re);
             __syncthreads();
-            fwd_f2<L>(prm.wtab, tid, reinterpret_cast<const float2 *>(s1),
-                      reinterpret_cast<float2 *>(s0));
+            fwd_f2<L>(prm.wtab, tid, s1.re, s0.re);
             __syncthreads();
-            fwd_f3<L>(tid, reinterpret_cast<const float2 *>(s0), xh);
+            fwd_f3<L>(tid, s0.re, xh);
             __syncthreads(); // s0 is rewritten by inv_q3 below
         }
         inv_q3<L>(xh, h4, tw, tid, s0);
@@ -317,53 +339,44 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
 
         const int row_p = pair;                         // z <= 0
         const int row_q = prm.ntemplates - 1 - pair;    // z >= 0 (same row for the z = 0 slot)
-        const bool has_q = row_q != row_p;
         const long long col0 = seg * prm.useful - prm.overlap;  // column of local index 0
         const bool interior = col0 + prm.overlap + prm.useful <= prm.nbins;
 
-        float2 p[16], q[16];
-        inv_q1<L>(tid, 0, s1, p, q);
+        cpk y[16];
+        inv_q1<L>(tid, 0, s1, y);
+        unsigned vm = vmask;
+        if (!interior) {
+#pragma unroll
+            for (int n1 = 0; n1 < 16; ++n1)
+                if (col0 + n1 * G::Q + tid >= prm.nbins) vm &= ~(1u << n1);
+        }
+        // The z = 0 slot has row_q == row_p and q == p bit for bit (H_0 is real), so its second
+        // store rewrites the same value: no special case.
         if constexpr (!INTERBIN) {
             float *bp = prm.plane + (size_t)row_p * prm.ncols + (col0 + tid);
             float *bq = prm.plane + (size_t)row_q * prm.ncols + (col0 + tid);
-            unsigned vm = vmask;
-            if (!interior) {
 #pragma unroll
-                for (int n1 = 0; n1 < 16; ++n1)
-                    if (col0 + n1 * G::Q + tid >= prm.nbins) vm &= ~(1u << n1);
-            }
-#pragma unroll
-            for (int n1 = 0; n1 < 16; ++n1)
-                if (vm & (1u << n1)) st_stream(bp + n1 * G::Q, power(p[n1]));
-            if (has_q) {
-#pragma unroll
-                for (int n1 = 0; n1 < 16; ++n1)
-                    if (vm & (1u << n1)) st_stream(bq + n1 * G::Q, power(q[n1]));
+            for (int n1 = 0; n1 < 16; ++n1) {
+                const float2 pw = power2(y[n1]);
+                st_stream_if(bp + n1 * G::Q, pw.x, vm & (1u << n1));
+                st_stream_if(bq + n1 * G::Q, pw.y, vm & (1u << n1));
             }
         } else {
 #pragma unroll
-            for (int n1 = 0; n1 < 16; ++n1)
-                s2[n1 * G::Q + tid] = make_float4(p[n1].x, p[n1].y, q[n1].x, q[n1].y);
+            for (int n1 = 0; n1 < 16; ++n1) s2.put(n1 * G::Q + tid, y[n1]);
             __syncthreads();
             float *bp = prm.plane + (size_t)row_p * prm.ncols + 2 * (col0 + tid);
             float *bq = prm.plane + (size_t)row_q * prm.ncols + 2 * (col0 + tid);
-            unsigned vm = vmask;
-            if (!interior) {
-#pragma unroll
-                for (int n1 = 0; n1 < 16; ++n1)
-                    if (col0 + n1 * G::Q + tid >= prm.nbins) vm &= ~(1u << n1);
-            }
 #pragma unroll
             for (int n1 = 0; n1 < 16; ++n1) {
-                if (vm & (1u << n1)) {
-                    const float4 nx = s2[n1 * G::Q + tid + 1]; // n + 1 <= overlap + useful < L
-                    const float2 dp = make_float2(p[n1].x - nx.x, p[n1].y - nx.y);
-                    st_stream2(bp + 2 * n1 * G::Q, power(p[n1]), IB * power(dp));
-                    if (has_q) {
-                        const float2 dq = make_float2(q[n1].x - nx.z, q[n1].y - nx.w);
-                        st_stream2(bq + 2 * n1 * G::Q, power(q[n1]), IB * power(dq));
-                    }
-                }
+                const cpk nx = s2.get(n1 * G::Q + tid + 1); // n + 1 <= overlap + useful < L
+                cpk d;
+                d.re = sub2(y[n1].re, nx.re);
+                d.im = sub2(y[n1].im, nx.im);
+                const float2 pw = power2(y[n1]);
+                const float2 ph = mul2(power2(d), bc2(IB));
+                st_stream2_if(bp + 2 * n1 * G::Q, pw.x, ph.x, vm & (1u << n1));
+                st_stream2_if(bq + 2 * n1 * G::Q, pw.y, ph.y, vm & (1u << n1));
             }
         }
         pair = npair;

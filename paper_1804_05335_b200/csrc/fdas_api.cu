@@ -7,6 +7,7 @@
 #include <atomic>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -43,18 +44,18 @@ namespace {
 
 typedef void (*kernel_fn)(const KernelParams);
 
-template <int L>
+template <int L, int MINB>
 kernel_fn pick_kernel(bool ib)
 {
-    return ib ? (kernel_fn)fdas_fused_kernel<L, true, 1> : (kernel_fn)fdas_fused_kernel<L, false, 1>;
+    return ib ? (kernel_fn)fdas_fused_kernel<L, true, MINB> : (kernel_fn)fdas_fused_kernel<L, false, MINB>;
 }
 
 kernel_fn select_kernel(int L, bool ib)
 {
     switch (L) {
-    case 1024: return pick_kernel<1024>(ib);
-    case 2048: return pick_kernel<2048>(ib);
-    case 4096: return pick_kernel<4096>(ib);
+    case 1024: return pick_kernel<1024, 4>(ib);
+    case 2048: return pick_kernel<2048, 2>(ib);
+    case 4096: return pick_kernel<4096, 1>(ib);
     default: return nullptr;
     }
 }
@@ -147,6 +148,9 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double
         if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)kern, I.threads,
                                                                I.smem_bytes)) != cudaSuccess) { st = FDAS_ERR_CUDA; break; }
         if (occ < 1) { st = FDAS_ERR_UNSUPPORTED; break; }
+#ifdef FDAS_TUNE
+        if (const char *e = getenv("FDAS_CTAS_PER_SM")) occ = atoi(e) < occ ? atoi(e) : occ;
+#endif
         I.ctas_per_sm = occ;
         I.grid = occ * I.sm_count;
         const size_t taps_bytes = (size_t)K * (2 * m + 1) * sizeof(double2);

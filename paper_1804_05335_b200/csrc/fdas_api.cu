@@ -62,8 +62,21 @@ kernel_fn select_kernel(int L, bool ib)
 
 int smem_bytes_for(int L, bool ib)
 {
-    const int e2 = L, e1 = 16 * (L / 16 + 1);
-    return (e2 + e1 + (ib ? L + 2 : 0)) * (int)sizeof(float4);
+    switch (L) {
+    case 1024: return Geo<1024>::smem_bytes(ib);
+    case 2048: return Geo<2048>::smem_bytes(ib);
+    case 4096: return Geo<4096>::smem_bytes(ib);
+    default: return 0;
+    }
+}
+
+void freq_to_reg_any(int L, int f, int &tid, int &i)
+{
+    switch (L) {
+    case 1024: freq_to_reg<1024>(f, tid, i); break;
+    case 2048: freq_to_reg<2048>(f, tid, i); break;
+    default: freq_to_reg<4096>(f, tid, i); break;
+    }
 }
 
 } // namespace
@@ -286,7 +299,7 @@ fdas_status fdas_get_template_spectrum(fdas_plan *p, int32_t k, float *host_re_i
     if (!p || !host_re_im || k < 0 || k >= p->info.ntemplates) return FDAS_ERR_INVALID_ARG;
     if (!p->ready) return FDAS_ERR_NOT_READY;
     const fdas_info &I = p->info;
-    const int L = I.seglen, T = L / 16, R3 = L / 256;
+    const int L = I.seglen, T = L / 16;
     const int pair = k < I.ntemplates - 1 - k ? k : I.ntemplates - 1 - k;
     const bool conj = k != pair;
     std::vector<float2> buf(L);
@@ -294,7 +307,8 @@ fdas_status fdas_get_template_spectrum(fdas_plan *p, int32_t k, float *host_re_i
     FDAS_CUDA(p, cudaMemcpy(buf.data(), p->d_hperm + (size_t)pair * L, (size_t)L * sizeof(float2),
                             cudaMemcpyDeviceToHost));
     for (int f = 0; f < L; ++f) {
-        const int b = f & 255, k3 = f >> 8, tid = b % T, i = (b / T) * R3 + k3;
+        int tid, i;
+        freq_to_reg_any(L, f, tid, i);
         const float2 v = buf[((size_t)(i >> 1) * T + tid) * 2 + (i & 1)];
         host_re_im[2 * f] = v.x;
         host_re_im[2 * f + 1] = conj ? -v.y : v.y; // H_{+z} = conj(H_{-z})

@@ -4,17 +4,28 @@
 // forward / DIT inverse, no re-ordering).  Everything between the segment load and the plane
 // store stays in registers and shared memory.
 //
-// Decomposition (L = 16 * 16 * R3, R3 = L/256; PTS = 16 points per thread, T = L/16 threads):
+// Decomposition (L = 16 * 16 * R3, R3 = L/256; PTS = 16 points per thread, T = L/16 threads,
+// W = T/32 warps, C = 16/W values of k1 owned by one warp):
 //   forward (DIF):  n = n1*(L/16) + n2*R3 + n3  ->  k = k1 + 16*k2 + 256*k3
-//     F1: DFT16 over n1 (thread <-> t1 = n2*R3+n3), twiddle W_L^{k1*t1}
-//     F2: DFT16 over n2 (thread <-> u  = k1 + 16*n3), twiddle W_L^{16*k2*n3}
-//     F3: DFT_R3 over n3 (thread <-> b = k1 + 16*k2, 16/R3 butterflies per thread)
+//     F1: DFT16 over n1 (thread <-> t1 = n2*R3+n3 = tid), twiddle W_L^{k1*t1}
+//     F2: DFT16 over n2 (thread <-> (k1, n3)),            twiddle W_L^{16*k2*n3}
+//     F3: DFT_R3 over n3 (thread <-> (k1, k2), 16/R3 butterflies per thread)
 //   inverse (DIT) is the exact mirror Q3, Q2, Q1 with conjugate twiddles, so the forward
 //   result X^ stays in registers in exactly the layout the inverse starts from, and the
 //   inverse ends with thread <-> output bin (coalesced plane stores).
-//   Exchange layouts (element units):  E2: k1 + 16*k2 + 256*n3       (size L)
-//                                      E1: k1*(L/16 + 1) + t1        (size L + 16, padded)
-//   Both are bank-conflict free for the 16-byte (+z, -z) element pairs of the inverse.
+//
+// Thread maps (w = warp, lane):
+//   F3/Q3: k1 = C*w + (lane % C), k2 = lane / C + (32/C)*j, j < 16/R3    (i = j*R3 + k3)
+//   F2/Q2: k1 = C*w + (lane % C), n3 = lane / C
+//   F1/Q1: t1 = tid
+// so the Q3 -> Q2 exchange (E2) never leaves the warp (only __syncwarp between them), and only
+// the Q2 -> Q1 exchange (E1) crosses warps.  E1 is double-buffered and guarded by one
+// split-phase mbarrier per buffer: a warp arrives after writing its Q2 results, runs Q3 of the
+// NEXT unit, and only then waits -- warps drift apart by up to a third of a unit, so one warp's
+// shared-memory phase overlaps another's FMA phase instead of all warps marching in lock step.
+//   E2 (per warp):  (lane%C) + C*n3 + (32+C)*k2          (512 + 15C elements, conflict-free)
+//   E1:             k1*(L/16 + 16/C) + t1                (conflict-free for both sides)
+// Elements are 16-byte (+z, -z) pairs split in two 8-byte planes (Re p, Re q) / (Im p, Im q).
 #pragma once
 #include "fdas_fft.cuh"
 #include <stdint.h>
@@ -25,16 +36,24 @@ template <int L>
 struct Geo {
     static constexpr int PTS = 16;           // points per thread per transform
     static constexpr int T = L / PTS;        // threads per CTA
+    static constexpr int W = T / 32;         // warps per CTA
+    static constexpr int C = 16 / W;         // k1 values per warp
+    static constexpr int KM = 32 / C;        // k2 values per Q3 butterfly index j
     static constexpr int R3 = L / 256;       // radix of the third pass
     static constexpr int NB3 = PTS / R3;     // R3-butterflies per thread in pass 3
-    static constexpr int NB2 = PTS / 16;     // 16-butterflies per thread in pass 2
-    static constexpr int NB1 = PTS / 16;     // 16-butterflies per thread in pass 1
     static constexpr int Q = L / 16;         // stride of n1 / number of t1 values
-    static constexpr int S1 = Q + 1;         // padded row length of exchange E1
-    static constexpr int E2_ELEMS = L;
+    static constexpr int S1 = Q + 16 / C;    // padded row length of exchange E1
+    static constexpr int S2 = 32 + C;        // k2 stride of the per-warp exchange E2
+    static constexpr int E2W = 512 + 15 * C;  // elements per warp region of E2
+    static constexpr int E2_ELEMS = W * E2W;
     static constexpr int E1_ELEMS = 16 * S1;
-    static constexpr int IB_ELEMS = L + 2;   // interbin neighbour exchange (index L is read, never used)
+    static constexpr int EDGE_ELEMS = 2 * 2 * W * 16;  // interbin: [buf][own|edge][warp][n1] float4
     static_assert(L == 1024 || L == 2048 || L == 4096, "segment length");
+    static_assert(NB3 * 2 == C && KM * NB3 == 16, "thread map");
+    static constexpr int smem_bytes(bool interbin)
+    {
+        return 16 /* two mbarriers */ + (E2_ELEMS + 2 * E1_ELEMS) * 16 + (interbin ? EDGE_ELEMS * 16 : 0);
+    }
 };
 
 // Index of X^'s frequency f in the per-thread register layout: returns (tid, i).
@@ -42,9 +61,11 @@ template <int L>
 FDAS_HD void freq_to_reg(int f, int &tid, int &i)
 {
     using G = Geo<L>;
-    const int b = f & 255, k3 = f >> 8;
-    tid = b % G::T;
-    i = (b / G::T) * G::R3 + k3;
+    const int k1 = f & 15, k2 = (f >> 4) & 15, k3 = f >> 8;
+    const int w = k1 / G::C, k1l = k1 % G::C;
+    const int j = k2 / G::KM, k2m = k2 % G::KM;
+    tid = 32 * w + k1l + G::C * k2m;
+    i = j * G::R3 + k3;
 }
 
 struct KernelParams {
@@ -61,59 +82,80 @@ struct KernelParams {
     int useful;               // B
 };
 
+// Per-thread constants of the thread maps above.
+template <int L>
+struct ThreadMap {
+    int tid, warp, lane;
+    int k1;        // F2/Q2 and F3/Q3
+    int n3;        // F2/Q2
+    int k2m;       // F3/Q3: k2 = k2m + KM*j
+    int e2_q3;     // E2 element index of (j = 0, n3 = 0) for this thread's Q3 butterflies
+    int e2_q2;     // E2 element index of k2 = 0 for this thread's Q2 butterfly
+    int e1_q2;     // E1 element index of n2 = 0 for this thread's Q2 butterfly
+    FDAS_HD explicit ThreadMap(int t)
+    {
+        using G = Geo<L>;
+        tid = t;
+        warp = t >> 5;
+        lane = t & 31;
+        const int k1l = lane % G::C;
+        k1 = G::C * warp + k1l;
+        n3 = lane / G::C;
+        k2m = lane / G::C;
+        e2_q3 = warp * G::E2W + k1l + G::S2 * k2m;
+        e2_q2 = warp * G::E2W + lane;
+        e1_q2 = k1 * G::S1 + n3;
+    }
+};
+
 // ------------------------------------------------------------------ forward passes (float2)
+// F1: load the segment (zero outside [0, nbins), reading R7), DFT16 over n1, twiddle, store E1.
 template <int L>
 FDAS_HD void fwd_f1(const float2 *__restrict__ spectrum, long long nbins, long long seg_start,
-                    const float2 *__restrict__ wtab, int tid, float2 *s1)
+                    const float2 *__restrict__ wtab, const ThreadMap<L> &tm, float2 *e1)
 {
     using G = Geo<L>;
+    const int t1 = tm.tid;
+    float2 a[16];
 #pragma unroll
-    for (int j = 0; j < G::NB1; ++j) {
-        const int t1 = tid + G::T * j;
-        float2 a[16];
+    for (int n1 = 0; n1 < 16; ++n1) {
+        const long long g = seg_start + n1 * G::Q + t1;
+        a[n1] = (g >= 0 && g < nbins) ? spectrum[g] : make_float2(0.f, 0.f);
+    }
+    dft<-1, 16>(a);
 #pragma unroll
-        for (int n1 = 0; n1 < 16; ++n1) {
-            const long long g = seg_start + n1 * G::Q + t1;
-            a[n1] = (g >= 0 && g < nbins) ? spectrum[g] : make_float2(0.f, 0.f);
-        }
-        dft<-1, 16>(a);
-#pragma unroll
-        for (int k1 = 0; k1 < 16; ++k1) {
-            const float2 v = (k1 == 0) ? a[0] : cmul(a[k1], wtab[(k1 * t1) & (L - 1)]);
-            s1[k1 * G::S1 + t1] = v;
-        }
+    for (int k1 = 0; k1 < 16; ++k1) {
+        const float2 v = (k1 == 0) ? a[0] : cmul(a[k1], wtab[(k1 * t1) & (L - 1)]);
+        e1[k1 * G::S1 + t1] = v;
     }
 }
 
+// F2: load E1 over n2, DFT16, twiddle, store E2 (this warp's region only).
 template <int L>
-FDAS_HD void fwd_f2(const float2 *__restrict__ wtab, int tid, const float2 *s1, float2 *s0)
+FDAS_HD void fwd_f2(const float2 *__restrict__ wtab, const ThreadMap<L> &tm, const float2 *e1, float2 *e2)
 {
     using G = Geo<L>;
+    float2 a[16];
 #pragma unroll
-    for (int j = 0; j < G::NB2; ++j) {
-        const int u = tid + G::T * j, k1 = u & 15, n3 = u >> 4;
-        float2 a[16];
+    for (int n2 = 0; n2 < 16; ++n2) a[n2] = e1[tm.e1_q2 + n2 * G::R3];
+    dft<-1, 16>(a);
 #pragma unroll
-        for (int n2 = 0; n2 < 16; ++n2) a[n2] = s1[k1 * G::S1 + n2 * G::R3 + n3];
-        dft<-1, 16>(a);
-#pragma unroll
-        for (int k2 = 0; k2 < 16; ++k2) {
-            const float2 v = (k2 == 0) ? a[0] : cmul(a[k2], wtab[16 * k2 * n3]);
-            s0[k1 + 16 * k2 + 256 * n3] = v;
-        }
+    for (int k2 = 0; k2 < 16; ++k2) {
+        const float2 v = (k2 == 0) ? a[0] : cmul(a[k2], wtab[16 * k2 * tm.n3]);
+        e2[tm.e2_q2 + G::S2 * k2] = v;
     }
 }
 
+// F3: load E2 over n3, DFT_R3 -> X^ in registers (i = j*R3 + k3).
 template <int L>
-FDAS_HD void fwd_f3(int tid, const float2 *s0, float2 (&xh)[Geo<L>::PTS])
+FDAS_HD void fwd_f3(const ThreadMap<L> &tm, const float2 *e2, float2 (&xh)[Geo<L>::PTS])
 {
     using G = Geo<L>;
 #pragma unroll
     for (int j = 0; j < G::NB3; ++j) {
-        const int b = tid + G::T * j;
         float2 a[G::R3];
 #pragma unroll
-        for (int n3 = 0; n3 < G::R3; ++n3) a[n3] = s0[b + 256 * n3];
+        for (int n3 = 0; n3 < G::R3; ++n3) a[n3] = e2[tm.e2_q3 + G::S2 * G::KM * j + G::C * n3];
         dft<-1, G::R3>(a);
 #pragma unroll
         for (int k3 = 0; k3 < G::R3; ++k3) xh[j * G::R3 + k3] = a[k3];
@@ -124,16 +166,16 @@ FDAS_HD void fwd_f3(int tid, const float2 *s0, float2 (&xh)[Geo<L>::PTS])
 template <int L>
 struct InvTwiddles {
     float2 tw3[Geo<L>::NB3][Geo<L>::R3]; // [j][n3]: exp(+2 pi i k2_j n3 / (16 R3)); n3 = 0 unused
-    float2 tw2[Geo<L>::NB2][16];         // [j][n2]: exp(+2 pi i k1 (n2 R3 + n3) / L)
+    float2 tw2[16];                      // [n2]: exp(+2 pi i k1 (n2 R3 + n3) / L)
 };
 
 template <int L>
-FDAS_HD void load_inv_twiddles(const float2 *__restrict__ wtab, int tid, InvTwiddles<L> &tw)
+FDAS_HD void load_inv_twiddles(const float2 *__restrict__ wtab, const ThreadMap<L> &tm, InvTwiddles<L> &tw)
 {
     using G = Geo<L>;
 #pragma unroll
     for (int j = 0; j < G::NB3; ++j) {
-        const int k2 = (tid + G::T * j) >> 4;
+        const int k2 = tm.k2m + G::KM * j;
 #pragma unroll
         for (int n3 = 0; n3 < G::R3; ++n3) {
             const float2 w = wtab[16 * k2 * n3];
@@ -141,13 +183,9 @@ FDAS_HD void load_inv_twiddles(const float2 *__restrict__ wtab, int tid, InvTwid
         }
     }
 #pragma unroll
-    for (int j = 0; j < G::NB2; ++j) {
-        const int u = tid + G::T * j, k1 = u & 15, n3 = u >> 4;
-#pragma unroll
-        for (int n2 = 0; n2 < 16; ++n2) {
-            const float2 w = wtab[k1 * (n2 * G::R3 + n3)];
-            tw.tw2[j][n2] = make_float2(w.x, -w.y);
-        }
+    for (int n2 = 0; n2 < 16; ++n2) {
+        const float2 w = wtab[tm.k1 * (n2 * G::R3 + tm.n3)];
+        tw.tw2[n2] = make_float2(w.x, -w.y);
     }
 }
 
@@ -158,7 +196,7 @@ __device__ __forceinline__ void load_h(const float4 *__restrict__ hp, int tid, f
 {
     using G = Geo<L>;
 #pragma unroll
-    for (int i2 = 0; i2 < G::PTS / 2; ++i2) h4[i2] = hp[i2 * G::T + tid];
+    for (int i2 = 0; i2 < G::PTS / 2; ++i2) h4[i2] = __ldg(hp + i2 * G::T + tid);
 }
 
 // Exchange buffer for packed pairs: the (Re p, Re q) and (Im p, Im q) register pairs live in two
@@ -182,17 +220,16 @@ struct XBuf {
 };
 
 // Q3: p = X^ * H, q = X^ * conj(H) as one packed pair, inverse DFT_R3 over k3,
-// twiddle, store E2.
+// twiddle, store E2 (this warp's region).
 //   (Re p, Re q) = x.re*h.re -+ x.im*h.im,   (Im p, Im q) = x.im*h.re +- x.re*h.im
 // (scalar FMUL/FFMA writing straight into the register pairs: 6 lane-ops per point).
 template <int L>
 __device__ __forceinline__ void inv_q3(const float2 (&xh)[Geo<L>::PTS], const float4 (&h4)[Geo<L>::PTS / 2],
-                                       const InvTwiddles<L> &tw, int tid, const XBuf &s0)
+                                       const InvTwiddles<L> &tw, const ThreadMap<L> &tm, const XBuf &e2)
 {
     using G = Geo<L>;
 #pragma unroll
     for (int j = 0; j < G::NB3; ++j) {
-        const int b = tid + G::T * j;
         cpk a[G::R3];
 #pragma unroll
         for (int k3 = 0; k3 < G::R3; ++k3) {
@@ -208,55 +245,41 @@ __device__ __forceinline__ void inv_q3(const float2 (&xh)[Geo<L>::PTS], const fl
 #pragma unroll
         for (int n3 = 0; n3 < G::R3; ++n3) {
             const cpk v = (n3 > 0) ? cmul(a[n3], tw.tw3[j][n3]) : a[n3];
-            s0.put(b + 256 * n3, v);
+            e2.put(tm.e2_q3 + G::S2 * G::KM * j + G::C * n3, v);
         }
     }
 }
 
-// Q2: load E2, inverse DFT16 over k2, twiddle, store E1.
+// Q2: load E2 (own warp's region), inverse DFT16 over k2, twiddle, store E1.
 template <int L>
-__device__ __forceinline__ void inv_q2(const InvTwiddles<L> &tw, int tid, const XBuf &s0, const XBuf &s1)
+__device__ __forceinline__ void inv_q2(const InvTwiddles<L> &tw, const ThreadMap<L> &tm, const XBuf &e2,
+                                       const XBuf &e1)
 {
     using G = Geo<L>;
+    cpk a[16];
 #pragma unroll
-    for (int j = 0; j < G::NB2; ++j) {
-        const int u = tid + G::T * j, k1 = u & 15, n3 = u >> 4;
-        cpk a[16];
+    for (int k2 = 0; k2 < 16; ++k2) a[k2] = e2.get(tm.e2_q2 + G::S2 * k2);
+    dft<+1, 16>(a);
 #pragma unroll
-        for (int k2 = 0; k2 < 16; ++k2) a[k2] = s0.get(k1 + 16 * k2 + 256 * n3);
-        dft<+1, 16>(a);
-#pragma unroll
-        for (int n2 = 0; n2 < 16; ++n2)
-            s1.put(k1 * G::S1 + n2 * G::R3 + n3, cmul(a[n2], tw.tw2[j][n2]));
-    }
+    for (int n2 = 0; n2 < 16; ++n2) e1.put(tm.e1_q2 + n2 * G::R3, cmul(a[n2], tw.tw2[n2]));
 }
 
-// Q1: load E1, inverse DFT16 over k1 -> y[n1*Q + t1] for butterfly j.
+// Q1: load E1, inverse DFT16 over k1 -> y[n1*Q + t1].
 template <int L>
-__device__ __forceinline__ void inv_q1(int tid, int j, const XBuf &s1, cpk (&a)[16])
+__device__ __forceinline__ void inv_q1(const ThreadMap<L> &tm, const XBuf &e1, cpk (&a)[16])
 {
     using G = Geo<L>;
-    const int t1 = tid + G::T * j;
 #pragma unroll
-    for (int k1 = 0; k1 < 16; ++k1) a[k1] = s1.get(k1 * G::S1 + t1);
+    for (int k1 = 0; k1 < 16; ++k1) a[k1] = e1.get(k1 * G::S1 + tm.tid);
     dft<+1, 16>(a);
 }
 
 // (|p|^2, |q|^2)
 __device__ __forceinline__ float2 power2(const cpk &y) { return fma2(y.im, y.im, mul2(y.re, y.re)); }
-#endif // __CUDACC__
-
-FDAS_HD float power(float2 y) { return y.x * y.x + y.y * y.y; }
-
-#ifdef __CUDACC__
 
 __device__ __forceinline__ void st_stream(float *p, float v)
 {
     asm volatile("st.global.cs.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory");
-}
-__device__ __forceinline__ void st_stream2(float *p, float a, float b)
-{
-    asm volatile("st.global.cs.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(a), "f"(b) : "memory");
 }
 // predicated forms (no branch around the store)
 __device__ __forceinline__ void st_stream_if(float *p, float v, unsigned pred)
@@ -270,6 +293,55 @@ __device__ __forceinline__ void st_stream2_if(float *p, float a, float b, unsign
                  ::"l"(p), "f"(a), "f"(b), "r"(pred) : "memory");
 }
 
+// ---- split-phase CTA barrier on shared memory (mbarrier): arrive now, wait later
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\t"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+                 "@!p bra WAIT_%=;\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+
+// Interbin cells whose neighbour y[n+1] lives in another warp (lane 31 of every warp) are finished
+// one unit late from the two small "own" / "edge" mailboxes written during Q1.
+template <int L>
+struct Pending {
+    long long col0;
+    int pair, par;
+    bool on;
+};
+
+template <int L>
+__device__ __forceinline__ void flush_edges(const KernelParams &prm, const ThreadMap<L> &tm, const float4 *edges,
+                                            Pending<L> &pd)
+{
+    using G = Geo<L>;
+    constexpr float IB = 0.61685027506808491367715568749226f; // (pi/4)^2, eq. 4 squared
+    const int n1 = tm.lane & 15;
+    const float4 *eb = edges + pd.par * (2 * G::W * 16);
+    const float4 a = eb[tm.warp * 16 + n1];                                   // y[n] of lane 31
+    const float4 b = (tm.warp < G::W - 1) ? eb[(G::W + tm.warp + 1) * 16 + n1]  // y[n+1]: next warp's lane 0
+                                          : eb[G::W * 16 + min(n1 + 1, 15)];    // ... or thread 0's next n1
+    const bool lo = tm.lane < 16;                                             // lanes 0-15: p row, 16-31: q row
+    const float dr = lo ? a.x - b.x : a.y - b.y;
+    const float di = lo ? a.z - b.z : a.w - b.w;
+    const float ph = IB * fmaf(di, di, dr * dr);
+    const int n = n1 * G::Q + 32 * tm.warp + 31;
+    const long long col = pd.col0 + n;
+    const int row = lo ? pd.pair : prm.ntemplates - 1 - pd.pair;
+    if (n >= prm.overlap && n < prm.overlap + prm.useful && col < prm.nbins)
+        st_stream(prm.plane + (size_t)row * prm.ncols + 2 * col + 1, ph);
+    pd.on = false;
+}
+
 // Persistent fused kernel.  Work = nseg * npairs (segment, template-slot) units, split into
 // gridDim.x equal contiguous ranges (segment-major), so each CTA redoes at most one extra
 // forward FFT at a range boundary and every CTA gets the same number of inverse FFT pairs.
@@ -278,74 +350,93 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
 {
     using G = Geo<L>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float2 *sm = reinterpret_cast<float2 *>(smem_raw);
-    const XBuf s0{sm, sm + G::E2_ELEMS};                                             // E2
-    const XBuf s1{sm + 2 * G::E2_ELEMS, sm + 2 * G::E2_ELEMS + G::E1_ELEMS};         // E1 (padded)
-    const XBuf s2{sm + 2 * (G::E2_ELEMS + G::E1_ELEMS),
-                  sm + 2 * (G::E2_ELEMS + G::E1_ELEMS) + G::IB_ELEMS};               // interbin only
-    const int tid = threadIdx.x;
+    uint64_t *mbar = reinterpret_cast<uint64_t *>(smem_raw);                 // full[0], full[1]
+    float2 *sm = reinterpret_cast<float2 *>(smem_raw + 16);
+    const XBuf e2{sm, sm + G::E2_ELEMS};                                     // per-warp regions
+    float2 *e1base = sm + 2 * G::E2_ELEMS;                                   // two (re, im) buffers
+    float4 *edges = reinterpret_cast<float4 *>(e1base + 4 * G::E1_ELEMS);    // interbin only
+    const ThreadMap<L> tm(threadIdx.x);
+    const int tid = tm.tid;
+
+    if (tid == 0) {
+        mbar_init(&mbar[0], G::T);
+        mbar_init(&mbar[1], G::T);
+    }
+    __syncthreads();
 
     InvTwiddles<L> tw;
-    load_inv_twiddles<L>(prm.wtab, tid, tw);
+    load_inv_twiddles<L>(prm.wtab, tm, tw);
 
     const long long units = prm.nseg * prm.npairs;
-    long long u = units * blockIdx.x / gridDim.x;
-    const long long u_end = units * (blockIdx.x + 1) / gridDim.x;
-    if (u >= u_end) return;
-    long long seg = u / prm.npairs;
-    int pair = (int)(u - seg * prm.npairs);
-    bool need_fwd = true;
+    const long long u0 = units * blockIdx.x / gridDim.x;
+    const int n = (int)(units * (blockIdx.x + 1) / gridDim.x - u0);
+    if (n <= 0) return;
+    long long seg = u0 / prm.npairs;
+    int pair = (int)(u0 - seg * prm.npairs);
+
     float2 xh[G::PTS];
     float4 h4[G::PTS / 2];
     constexpr size_t HSTRIDE = (size_t)(G::PTS / 2) * G::T;
-    load_h<L>(prm.hperm + pair * HSTRIDE, tid, h4);
+    int hnext = pair, hloaded = 0;                // H is fetched one unit ahead, in unit order
+    auto fetch_h = [&]() {
+        if (hloaded < n) {
+            load_h<L>(prm.hperm + hnext * HSTRIDE, tid, h4);
+            ++hloaded;
+            hnext = (hnext + 1 == prm.npairs) ? 0 : hnext + 1;
+        }
+    };
+    fetch_h();
 
     // which of this thread's 16 outputs n = n1*Q + tid fall in the useful range [ov, ov+B)
-    static_assert(G::NB1 == 1, "epilogue assumes one Q1 butterfly per thread");
     unsigned vmask = 0;
 #pragma unroll
     for (int n1 = 0; n1 < 16; ++n1) {
-        const int n = n1 * G::Q + tid;
-        if (n >= prm.overlap && n < prm.overlap + prm.useful) vmask |= 1u << n1;
+        const int nn = n1 * G::Q + tid;
+        if (nn >= prm.overlap && nn < prm.overlap + prm.useful) vmask |= 1u << n1;
     }
 
     constexpr float IB = 0.61685027506808491367715568749226f; // (pi/4)^2, eq. 4 squared
+    Pending<L> pend{0, 0, 0, false};
+    bool have_q3 = false;
 
-    for (; u < u_end; ++u) {
-        if (need_fwd) {
-            need_fwd = false;
-            __syncthreads(); // previous unit's readers of s1 are done
-            fwd_f1<L>(prm.spectrum, prm.nbins, seg * prm.useful - prm.overlap, prm.wtab, tid, s1.re);
+    for (int c = 0; c < n; ++c) {
+        if (!have_q3) {
+            // first unit of a segment for this CTA: the pipeline is drained; forward transform
+            __syncthreads();                                  // nobody reads E1 / E2 / edges any more
+            if (INTERBIN && pend.on) flush_edges<L>(prm, tm, edges, pend);
+            fwd_f1<L>(prm.spectrum, prm.nbins, seg * prm.useful - prm.overlap, prm.wtab, tm, e1base);
             __syncthreads();
-            fwd_f2<L>(prm.wtab, tid, s1.re, s0.re);
-            __syncthreads();
-            fwd_f3<L>(tid, s0.re, xh);
-            __syncthreads(); // s0 is rewritten by inv_q3 below
+            fwd_f2<L>(prm.wtab, tm, e1base, e2.re);
+            __syncwarp();
+            fwd_f3<L>(tm, e2.re, xh);
+            __syncthreads();                                  // E1[0] is rewritten by Q2 below
+            inv_q3<L>(xh, h4, tw, tm, e2);
+            fetch_h();
+            __syncwarp();
         }
-        inv_q3<L>(xh, h4, tw, tid, s0);
-        __syncthreads();
+        const int par = c & 1;
+        const XBuf e1{e1base + par * 2 * G::E1_ELEMS, e1base + par * 2 * G::E1_ELEMS + G::E1_ELEMS};
+        inv_q2<L>(tw, tm, e2, e1);
+        mbar_arrive(&mbar[par]);                              // this warp's share of E1[par] is written
+        __syncwarp();                                         // ... and its reads of E2 are done
 
-        // next unit; its H is fetched now so the L2 latency hides behind Q2/Q1
-        int npair = pair + 1;
-        long long nseg_ = seg;
-        if (npair == prm.npairs) {
-            npair = 0;
-            ++nseg_;
+        // Q3 of the next unit (same segment) fills the time until the other warps arrive
+        have_q3 = (c + 1 < n) && (pair + 1 < prm.npairs);
+        if (have_q3) {
+            inv_q3<L>(xh, h4, tw, tm, e2);
+            fetch_h();
         }
-        if (u + 1 < u_end) load_h<L>(prm.hperm + npair * HSTRIDE, tid, h4);
+        mbar_wait(&mbar[par], (c >> 1) & 1);                  // all of E1[par] is written
 
-        inv_q2<L>(tw, tid, s0, s1);
-        __syncthreads();
+        if (INTERBIN && pend.on) flush_edges<L>(prm, tm, edges, pend);   // every warp is past Q1(c-1)
 
         const int row_p = pair;                         // z <= 0
         const int row_q = prm.ntemplates - 1 - pair;    // z >= 0 (same row for the z = 0 slot)
         const long long col0 = seg * prm.useful - prm.overlap;  // column of local index 0
-        const bool interior = col0 + prm.overlap + prm.useful <= prm.nbins;
-
         cpk y[16];
-        inv_q1<L>(tid, 0, s1, y);
+        inv_q1<L>(tm, e1, y);
         unsigned vm = vmask;
-        if (!interior) {
+        if (col0 + prm.overlap + prm.useful > prm.nbins) {
 #pragma unroll
             for (int n1 = 0; n1 < 16; ++n1)
                 if (col0 + n1 * G::Q + tid >= prm.nbins) vm &= ~(1u << n1);
@@ -362,28 +453,49 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
                 st_stream_if(bq + n1 * G::Q, pw.y, vm & (1u << n1));
             }
         } else {
+            float4 *eb = edges + par * (2 * G::W * 16);
+            if (tm.lane == 31) {
 #pragma unroll
-            for (int n1 = 0; n1 < 16; ++n1) s2.put(n1 * G::Q + tid, y[n1]);
-            __syncthreads();
+                for (int n1 = 0; n1 < 16; ++n1)
+                    eb[tm.warp * 16 + n1] = make_float4(y[n1].re.x, y[n1].re.y, y[n1].im.x, y[n1].im.y);
+            }
+            if (tm.lane == 0) {
+#pragma unroll
+                for (int n1 = 0; n1 < 16; ++n1)
+                    eb[(G::W + tm.warp) * 16 + n1] = make_float4(y[n1].re.x, y[n1].re.y, y[n1].im.x, y[n1].im.y);
+            }
             float *bp = prm.plane + (size_t)row_p * prm.ncols + 2 * (col0 + tid);
             float *bq = prm.plane + (size_t)row_q * prm.ncols + 2 * (col0 + tid);
+            const unsigned last = tm.lane == 31;
 #pragma unroll
             for (int n1 = 0; n1 < 16; ++n1) {
-                const cpk nx = s2.get(n1 * G::Q + tid + 1); // n + 1 <= overlap + useful < L
-                cpk d;
-                d.re = sub2(y[n1].re, nx.re);
-                d.im = sub2(y[n1].im, nx.im);
+                cpk d;                                   // y[n] - y[n+1], neighbour from lane + 1
+                d.re = sub2(y[n1].re, make_float2(__shfl_down_sync(0xffffffffu, y[n1].re.x, 1),
+                                                  __shfl_down_sync(0xffffffffu, y[n1].re.y, 1)));
+                d.im = sub2(y[n1].im, make_float2(__shfl_down_sync(0xffffffffu, y[n1].im.x, 1),
+                                                  __shfl_down_sync(0xffffffffu, y[n1].im.y, 1)));
                 const float2 pw = power2(y[n1]);
                 const float2 ph = mul2(power2(d), bc2(IB));
-                st_stream2_if(bp + 2 * n1 * G::Q, pw.x, ph.x, vm & (1u << n1));
-                st_stream2_if(bq + 2 * n1 * G::Q, pw.y, ph.y, vm & (1u << n1));
+                const unsigned v = (vm >> n1) & 1u;
+                st_stream2_if(bp + 2 * n1 * G::Q, pw.x, ph.x, v & ~last);
+                st_stream2_if(bq + 2 * n1 * G::Q, pw.y, ph.y, v & ~last);
+                st_stream_if(bp + 2 * n1 * G::Q, pw.x, v & last);   // half-bin follows in flush_edges
+                st_stream_if(bq + 2 * n1 * G::Q, pw.y, v & last);
             }
+            pend.col0 = col0;
+            pend.pair = pair;
+            pend.par = par;
+            pend.on = true;
         }
-        pair = npair;
-        if (nseg_ != seg) {
-            seg = nseg_;
-            need_fwd = true;
+        __syncwarp();
+        if (++pair == prm.npairs) {
+            pair = 0;
+            ++seg;
         }
+    }
+    if (INTERBIN && pend.on) {
+        __syncthreads();
+        flush_edges<L>(prm, tm, edges, pend);
     }
 }
 

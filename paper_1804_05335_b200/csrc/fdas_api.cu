@@ -22,7 +22,8 @@ struct fdas_plan {
     bool ready;
     double2 *d_taps;     // K x (2m+1)
     float2 *d_hperm;     // npairs x L (kernel register order)
-    float2 *d_wtab;      // L
+    float2 *d_wtab;      // L (seglen 8192: the 4096 table)
+    float2 *d_wtab2;     // seglen 8192 only: 8192 entries
     float2 *d_stage_in;  // fdas_execute_host staging (lazy)
     float *d_stage_out;
     void (*kernel)(const KernelParams);
@@ -56,6 +57,7 @@ kernel_fn select_kernel(int L, bool ib)
     case 1024: return pick_kernel<1024, 4>(ib);
     case 2048: return pick_kernel<2048, 2>(ib);
     case 4096: return pick_kernel<4096, 1>(ib);
+    case 8192: return ib ? nullptr : (kernel_fn)fdas_fused_kernel_8k<1>;   // 2 x 4096, no interbin
     default: return nullptr;
     }
 }
@@ -66,6 +68,7 @@ int smem_bytes_for(int L, bool ib)
     case 1024: return Geo<1024>::smem_bytes(ib);
     case 2048: return Geo<2048>::smem_bytes(ib);
     case 4096: return Geo<4096>::smem_bytes(ib);
+    case 8192: return Geo8k::smem_bytes();
     default: return 0;
     }
 }
@@ -75,7 +78,7 @@ void freq_to_reg_any(int L, int f, int &tid, int &i)
     switch (L) {
     case 1024: freq_to_reg<1024>(f, tid, i); break;
     case 2048: freq_to_reg<2048>(f, tid, i); break;
-    default: freq_to_reg<4096>(f, tid, i); break;
+    default: freq_to_reg<4096>(f & 4095, tid, i); break;   // 8192: slot of f mod 4096 in half f / 4096
     }
 }
 
@@ -142,7 +145,7 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double
     I.useful = B;
     I.interbin = interbin;
     I.npairs = (K + 1) / 2;
-    I.threads = seglen / 16;
+    I.threads = seglen == 8192 ? 256 : seglen / 16;
     I.smem_bytes = smem_bytes_for(seglen, interbin != 0);
 
     fdas_status st = FDAS_OK;
@@ -170,7 +173,8 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double
         const size_t h_bytes = (size_t)I.npairs * seglen * sizeof(float2);
         if (cudaMalloc(&p->d_taps, taps_bytes) != cudaSuccess ||
             cudaMalloc(&p->d_hperm, h_bytes) != cudaSuccess ||
-            cudaMalloc(&p->d_wtab, (size_t)seglen * sizeof(float2)) != cudaSuccess) {
+            cudaMalloc(&p->d_wtab, (size_t)seglen * sizeof(float2)) != cudaSuccess ||
+            (seglen == 8192 && cudaMalloc(&p->d_wtab2, (size_t)seglen * sizeof(float2)) != cudaSuccess)) {
             cudaGetLastError();
             st = FDAS_ERR_NOMEM;
             break;
@@ -193,13 +197,19 @@ fdas_status fdas_make_templates(fdas_plan *p, void *stream)
     {
         const int n = I.ntemplates * w;
         make_taps_kernel<<<(n + 127) / 128, 128, 0, st>>>(p->d_taps, I.ntemplates, I.halfwidth, I.zmax, I.dz);
-        make_wtab_kernel<<<(I.seglen + 127) / 128, 128, 0, st>>>(p->d_wtab, I.seglen);
+        const int lw = I.seglen == 8192 ? 4096 : I.seglen;   // table of the kernel's passes
+        make_wtab_kernel<<<(lw + 127) / 128, 128, 0, st>>>(p->d_wtab, lw);
+        if (I.seglen == 8192) {
+            make_wtab_kernel<<<(8192 + 127) / 128, 128, 0, st>>>(p->d_wtab2, 8192);
+            g_launches += 1;
+        }
         const int nh = I.npairs * I.seglen;
         const int gb = (nh + 127) / 128;
         switch (I.seglen) {
         case 1024: make_spectra_kernel<1024><<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps, I.npairs, I.halfwidth, I.zmax, I.dz, I.ntemplates); break;
         case 2048: make_spectra_kernel<2048><<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps, I.npairs, I.halfwidth, I.zmax, I.dz, I.ntemplates); break;
         case 4096: make_spectra_kernel<4096><<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps, I.npairs, I.halfwidth, I.zmax, I.dz, I.ntemplates); break;
+        case 8192: make_spectra_kernel_8k<<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps, I.npairs, I.halfwidth, I.zmax, I.dz, I.ntemplates); break;
         default: return FDAS_ERR_UNSUPPORTED;
         }
         g_launches += 3;
@@ -220,6 +230,7 @@ fdas_status fdas_execute(fdas_plan *p, void *stream, const void *d_spectrum, flo
     prm.plane = d_plane;
     prm.hperm = (const float4 *)p->d_hperm;
     prm.wtab = p->d_wtab;
+    prm.wtab2 = p->d_wtab2;
     prm.nbins = I.nbins;
     prm.ncols = I.ncols;
     prm.nseg = I.nseg;
@@ -264,6 +275,7 @@ fdas_status fdas_destroy(fdas_plan *p)
     cudaFree(p->d_taps);
     cudaFree(p->d_hperm);
     cudaFree(p->d_wtab);
+    cudaFree(p->d_wtab2);
     cudaFree(p->d_stage_in);
     cudaFree(p->d_stage_out);
     cudaGetLastError();
@@ -299,7 +311,7 @@ fdas_status fdas_get_template_spectrum(fdas_plan *p, int32_t k, float *host_re_i
     if (!p || !host_re_im || k < 0 || k >= p->info.ntemplates) return FDAS_ERR_INVALID_ARG;
     if (!p->ready) return FDAS_ERR_NOT_READY;
     const fdas_info &I = p->info;
-    const int L = I.seglen, T = L / 16;
+    const int L = I.seglen, T = I.threads;
     const int pair = k < I.ntemplates - 1 - k ? k : I.ntemplates - 1 - k;
     const bool conj = k != pair;
     std::vector<float2> buf(L);
@@ -309,7 +321,8 @@ fdas_status fdas_get_template_spectrum(fdas_plan *p, int32_t k, float *host_re_i
     for (int f = 0; f < L; ++f) {
         int tid, i;
         freq_to_reg_any(L, f, tid, i);
-        const float2 v = buf[((size_t)(i >> 1) * T + tid) * 2 + (i & 1)];
+        const size_t half = (L == 8192) ? (size_t)(f >> 12) * 4096 : 0;   // [half][i/2][tid]
+        const float2 v = buf[half + ((size_t)(i >> 1) * T + tid) * 2 + (i & 1)];
         host_re_im[2 * f] = v.x;
         host_re_im[2 * f + 1] = conj ? -v.y : v.y; // H_{+z} = conj(H_{-z})
     }

@@ -72,7 +72,8 @@ struct KernelParams {
     const float2 *spectrum;   // N complex64
     float *plane;             // K x ncols
     const float4 *hperm;      // [npairs][PTS/2][T] float4 = 2 complex H values (z <= 0 rows)
-    const float2 *wtab;       // exp(-2 pi i j / L), j < L
+    const float2 *wtab;       // exp(-2 pi i j / L), j < L   (seglen 8192: L = 4096 here)
+    const float2 *wtab2;      // seglen 8192 only: exp(-2 pi i j / 8192), j < 8192
     long long nbins;
     long long ncols;
     long long nseg;
@@ -110,7 +111,8 @@ struct ThreadMap {
 
 // ------------------------------------------------------------------ forward passes (float2)
 // F1: load the segment (zero outside [0, nbins), reading R7), DFT16 over n1, twiddle, store E1.
-template <int L>
+// STRIDE/OFF: the transform's input n is bin seg_start + STRIDE*n + OFF (8192 = 2 x 4096 path).
+template <int L, int STRIDE = 1, int OFF = 0>
 FDAS_HD void fwd_f1(const float2 *__restrict__ spectrum, long long nbins, long long seg_start,
                     const float2 *__restrict__ wtab, const ThreadMap<L> &tm, float2 *e1)
 {
@@ -119,7 +121,7 @@ FDAS_HD void fwd_f1(const float2 *__restrict__ spectrum, long long nbins, long l
     float2 a[16];
 #pragma unroll
     for (int n1 = 0; n1 < 16; ++n1) {
-        const long long g = seg_start + n1 * G::Q + t1;
+        const long long g = seg_start + STRIDE * (n1 * G::Q + t1) + OFF;
         a[n1] = (g >= 0 && g < nbins) ? spectrum[g] : make_float2(0.f, 0.f);
     }
     dft<-1, 16>(a);

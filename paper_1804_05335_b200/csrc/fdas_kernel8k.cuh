@@ -1,0 +1,231 @@
+// Fused FDAS kernel for segment length 8192 = 2 x 4096 (BASELINE config 4).
+//
+// A 16-point-per-thread CTA for 8192 points would need 512 threads x <= 128 registers and two
+// 128 KB exchange buffers; neither fits.  Instead the 4096-point machinery of fdas_kernel.cuh
+// (256 threads, Geo<4096>) runs twice per template slot:
+//
+//   forward, once per segment (decimation in time over the INPUT parity):
+//       Ee = DFT_4096(x[2n]),  Oo = DFT_4096(x[2n+1]),   W = exp(-2 pi i / 8192)
+//       X^[k] = Ee[k] + W^k Oo[k],   X^[k+4096] = Ee[k] - W^k Oo[k],   k < 4096
+//     both halves go to a thread-private 64 KB shared-memory array (slot order of Geo<4096>).
+//   inverse, per (slot, parity pi) sub-unit (decimation in frequency over the OUTPUT parity):
+//       y[2n'+pi] = IDFT_4096( ( (X^H)[k] + (-1)^pi (X^H)[k+4096] ) conj(W)^(pi k) )[n']
+//     the Q3 input stage forms the two products (for H and conj H), their sum or
+//     twiddled difference, then Q3/Q2/Q1 run as in the 4096 kernel.  H (both halves, 64
+//     registers) is loaded once per slot and serves both parities.
+//   store: column 2n'+pi of rows -|z| and +|z| (stride-2 streaming stores; the two parities of
+//     a slot follow each other in the same CTA, so L2 merges the sectors).
+//
+// With X^ in shared memory only ONE E1 buffer fits: the split-phase `full` barrier is paired
+// with an `empty` barrier (arrive after Q1's loads, wait before Q2's stores).
+#pragma once
+#include "fdas_kernel.cuh"
+
+namespace fdas {
+
+struct Geo8k {
+    using G = Geo<4096>;
+    static constexpr int L = 8192;
+    static constexpr int XS_ELEMS = 2 * G::PTS * G::T; // float2: X^lo[16][T], X^hi[16][T]
+    static constexpr int smem_bytes() { return 32 + (G::E2_ELEMS + G::E1_ELEMS) * 16 + XS_ELEMS * 8; }
+};
+
+#ifdef __CUDACC__
+
+// exp(+2 pi i i / 32), i < 16
+__device__ __forceinline__ constexpr float c32re(int i) { return cosw(i); }
+__device__ __forceinline__ constexpr float c32im(int i) { return sinw(i); }
+
+// Q3 of one parity: products, sum / twiddled difference, inverse DFT16 over k3, twiddle, store E2.
+template <int PARITY>
+__device__ __forceinline__ void inv_q3_8k(const float2 *xs_lo, const float2 *xs_hi, const float4 (&hlo)[8],
+                                          const float4 (&hhi)[8], float2 wb, const InvTwiddles<4096> &tw,
+                                          const ThreadMap<4096> &tm, const XBuf &e2)
+{
+    using G = Geo<4096>;
+    cpk a[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        const float2 xl = xs_lo[i * G::T + tm.tid], xh = xs_hi[i * G::T + tm.tid];
+        const float4 l4 = hlo[i >> 1], h4 = hhi[i >> 1];
+        const float2 hl = (i & 1) ? make_float2(l4.z, l4.w) : make_float2(l4.x, l4.y);
+        const float2 hh = (i & 1) ? make_float2(h4.z, h4.w) : make_float2(h4.x, h4.y);
+        constexpr float sg = PARITY ? -1.0f : 1.0f;
+        // p = xl hl + sg xh hh,  q = xl conj(hl) + sg xh conj(hh)
+        const float ac = fmaf(sg * xh.x, hh.x, xl.x * hl.x);
+        const float bd = fmaf(sg * xh.y, hh.y, xl.y * hl.y);
+        const float bc = fmaf(sg * xh.y, hh.x, xl.y * hl.x);
+        const float ad = fmaf(sg * xh.x, hh.y, xl.x * hl.y);
+        cpk v;
+        v.re = make_float2(ac - bd, ac + bd);
+        v.im = make_float2(bc + ad, bc - ad);
+        if constexpr (PARITY) {
+            v = cmul(v, wb);                                   // conj(W)^(k1 + 16 k2)
+        }
+        a[i] = v;
+    }
+    if constexpr (PARITY) {
+        // conj(W)^(256 i) = exp(+2 pi i i / 32): compile-time constants
+#pragma unroll
+        for (int i = 1; i < 16; ++i) a[i] = cmul(a[i], make_float2(c32re(i), c32im(i)));
+    }
+    dft<+1, 16>(a);
+#pragma unroll
+    for (int n3 = 0; n3 < 16; ++n3) {
+        const cpk v = (n3 > 0) ? cmul(a[n3], tw.tw3[0][n3]) : a[n3];
+        e2.put(tm.e2_q3 + G::C * n3, v);
+    }
+}
+
+template <int MINB>
+__global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelParams prm)
+{
+    using G = Geo<4096>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    uint64_t *mbar = reinterpret_cast<uint64_t *>(smem_raw);                 // [0] full, [1] empty
+    float2 *sm = reinterpret_cast<float2 *>(smem_raw + 32);
+    const XBuf e2{sm, sm + G::E2_ELEMS};
+    float2 *e1base = sm + 2 * G::E2_ELEMS;
+    const XBuf e1{e1base, e1base + G::E1_ELEMS};
+    float2 *xs_lo = e1base + 2 * G::E1_ELEMS;
+    float2 *xs_hi = xs_lo + G::PTS * G::T;
+    const ThreadMap<4096> tm(threadIdx.x);
+    const int tid = tm.tid;
+
+    if (tid == 0) {
+        mbar_init(&mbar[0], G::T);
+        mbar_init(&mbar[1], G::T);
+    }
+    __syncthreads();
+
+    InvTwiddles<4096> tw;
+    load_inv_twiddles<4096>(prm.wtab, tm, tw);
+    // conj(W_8192)^(k1 + 16 k2) for this thread's Q3 slots
+    float2 wb;
+    {
+        const float2 w = prm.wtab2[tm.k1 + 16 * tm.k2m];
+        wb = make_float2(w.x, -w.y);
+    }
+
+    const long long units = prm.nseg * prm.npairs;
+    const long long u0 = units * blockIdx.x / gridDim.x;
+    const int n = (int)(units * (blockIdx.x + 1) / gridDim.x - u0);
+    if (n <= 0) return;
+    long long seg = u0 / prm.npairs;
+    int pair = (int)(u0 - seg * prm.npairs);
+
+    float4 hlo[8], hhi[8];
+    constexpr size_t HSTRIDE = (size_t)8 * G::T;      // float4 per half
+    int hnext = pair, hloaded = 0;
+    auto fetch_h = [&]() {
+        if (hloaded < n) {
+            const float4 *hp = prm.hperm + (size_t)hnext * 2 * HSTRIDE;
+#pragma unroll
+            for (int i2 = 0; i2 < 8; ++i2) hlo[i2] = __ldg(hp + i2 * G::T + tid);
+#pragma unroll
+            for (int i2 = 0; i2 < 8; ++i2) hhi[i2] = __ldg(hp + HSTRIDE + i2 * G::T + tid);
+            ++hloaded;
+            hnext = (hnext + 1 == prm.npairs) ? 0 : hnext + 1;
+        }
+    };
+    fetch_h();
+
+    // useful outputs in units of n' (n = 2n' + parity; overlap and useful are even)
+    const int ov2 = prm.overlap >> 1, us2 = prm.useful >> 1;
+    unsigned vmask = 0;
+#pragma unroll
+    for (int n1 = 0; n1 < 16; ++n1) {
+        const int nn = n1 * G::Q + tid;
+        if (nn >= ov2 && nn < ov2 + us2) vmask |= 1u << n1;
+    }
+
+    bool have_q3 = false;
+    const int nsub = 2 * n;
+    for (int c = 0; c < nsub; ++c) {
+        const int par = c & 1;
+        if (!have_q3) {
+            // first sub-unit of a segment for this CTA (always parity 0): forward transform
+            __syncthreads();
+            const long long g0 = seg * prm.useful - prm.overlap;
+            float2 xe[16], xo[16];
+            fwd_f1<4096, 2, 0>(prm.spectrum, prm.nbins, g0, prm.wtab, tm, e1base);
+            __syncthreads();
+            fwd_f2<4096>(prm.wtab, tm, e1base, e2.re);
+            __syncwarp();
+            fwd_f3<4096>(tm, e2.re, xe);
+            __syncthreads();
+            fwd_f1<4096, 2, 1>(prm.spectrum, prm.nbins, g0, prm.wtab, tm, e1base);
+            __syncthreads();
+            fwd_f2<4096>(prm.wtab, tm, e1base, e2.re);
+            __syncwarp();
+            fwd_f3<4096>(tm, e2.re, xo);
+            __syncthreads();                                   // E1 / E2 are rewritten below
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                const float2 t = cmul(xo[i], prm.wtab2[tm.k1 + 16 * tm.k2m + 256 * i]);
+                xs_lo[i * G::T + tid] = cadd(xe[i], t);        // thread-private slots
+                xs_hi[i * G::T + tid] = csub(xe[i], t);
+            }
+            inv_q3_8k<0>(xs_lo, xs_hi, hlo, hhi, wb, tw, tm, e2);
+            __syncwarp();
+        }
+        // Q2: load E2, inverse DFT16 over k2, twiddle; E1 must be free before the stores
+        {
+            cpk a[16];
+#pragma unroll
+            for (int k2 = 0; k2 < 16; ++k2) a[k2] = e2.get(tm.e2_q2 + G::S2 * k2);
+            dft<+1, 16>(a);
+#pragma unroll
+            for (int n2 = 0; n2 < 16; ++n2) a[n2] = cmul(a[n2], tw.tw2[n2]);
+            if (c > 0) mbar_wait(&mbar[1], (c - 1) & 1);       // every warp has loaded Q1(c-1)
+#pragma unroll
+            for (int n2 = 0; n2 < 16; ++n2) e1.put(tm.e1_q2 + n2 * G::R3, a[n2]);
+        }
+        mbar_arrive(&mbar[0]);
+        __syncwarp();
+
+        // Q3 of the next sub-unit of the same segment
+        have_q3 = (c + 1 < nsub) && (par == 0 || pair + 1 < prm.npairs);
+        if (have_q3) {
+            if (par == 0) {
+                inv_q3_8k<1>(xs_lo, xs_hi, hlo, hhi, wb, tw, tm, e2);
+                fetch_h();                                     // next slot's H, one sub-unit ahead
+            } else {
+                inv_q3_8k<0>(xs_lo, xs_hi, hlo, hhi, wb, tw, tm, e2);
+            }
+        }
+        mbar_wait(&mbar[0], c & 1);
+
+        const int row_p = pair;
+        const int row_q = prm.ntemplates - 1 - pair;
+        const long long col0 = seg * prm.useful - prm.overlap;
+        cpk y[16];
+#pragma unroll
+        for (int k1 = 0; k1 < 16; ++k1) y[k1] = e1.get(k1 * G::S1 + tid);
+        mbar_arrive(&mbar[1]);                                 // E1 may be overwritten
+        dft<+1, 16>(y);
+        unsigned vm = vmask;
+        if (col0 + prm.overlap + prm.useful > prm.nbins) {
+#pragma unroll
+            for (int n1 = 0; n1 < 16; ++n1)
+                if (col0 + 2 * (n1 * G::Q + tid) + par >= prm.nbins) vm &= ~(1u << n1);
+        }
+        float *bp = prm.plane + (size_t)row_p * prm.ncols + (col0 + 2 * tid + par);
+        float *bq = prm.plane + (size_t)row_q * prm.ncols + (col0 + 2 * tid + par);
+#pragma unroll
+        for (int n1 = 0; n1 < 16; ++n1) {
+            const float2 pw = power2(y[n1]);
+            st_stream_if(bp + 2 * n1 * G::Q, pw.x, vm & (1u << n1));
+            st_stream_if(bq + 2 * n1 * G::Q, pw.y, vm & (1u << n1));
+        }
+        __syncwarp();
+        if (par == 1 && ++pair == prm.npairs) {
+            pair = 0;
+            ++seg;
+        }
+    }
+}
+
+#endif // __CUDACC__
+
+} // namespace fdas

@@ -11,6 +11,7 @@
 //      written in the register order of the fused kernel's un-permuted FFT.
 #pragma once
 #include "fdas_kernel.cuh"
+#include "fdas_kernel8k.cuh"
 
 namespace fdas {
 
@@ -138,6 +139,37 @@ __global__ void make_spectra_kernel(float2 *hperm, const double2 *taps, int npai
     int tid, i;
     freq_to_reg<L>(f, tid, i);
     const size_t off = (((size_t)pair * (G::PTS / 2) + (i >> 1)) * G::T + tid) * 2 + (i & 1);
+    hperm[off] = make_float2((float)(sr / L), (float)(si / L));
+}
+
+// seglen 8192: hperm[pair][half][i/2][tid] with half 0 = H[k], half 1 = H[k + 4096], k < 4096 in
+// the slot order of Geo<4096> (fdas_kernel8k.cuh).
+__global__ void make_spectra_kernel_8k(float2 *hperm, const double2 *taps, int npairs, int m,
+                                       double zmax, double dz, int K)
+{
+    using G = Geo<4096>;
+    constexpr int L = 8192;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= npairs * L) return;
+    const int pair = idx / L, f = idx % L;
+    const int center = (K - 1) / 2;
+    const double z = (pair == center) ? 0.0 : -zmax + pair * dz;
+    const int mz = tap_halfwidth(z);
+    const double2 *h = taps + (size_t)pair * (2 * m + 1) + m;
+    double sr = 0.0, si = 0.0;
+    for (int d = -mz; d <= mz; ++d) {
+        int r = (int)(((long long)d * f) % L);
+        if (r < 0) r += L;
+        double s, c;
+        sincospi(2.0 * r / L, &s, &c);
+        const double2 t = h[d];
+        sr += t.x * c + t.y * s;
+        si += t.x * s - t.y * c;
+    }
+    int tid, i;
+    freq_to_reg<4096>(f & 4095, tid, i);
+    const int half = f >> 12;
+    const size_t off = ((((size_t)pair * 2 + half) * (G::PTS / 2) + (i >> 1)) * G::T + tid) * 2 + (i & 1);
     hperm[off] = make_float2((float)(sr / L), (float)(si / L));
 }
 

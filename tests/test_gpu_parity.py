@@ -72,7 +72,7 @@ def check_rows(orc, spectrum, plane, zmax, dz, interbin, rows=None):
 
 # ------------------------------------------------------------------ templates (a0, a1)
 @pytest.mark.parametrize("zmax,dz,seglen", [(20.0, 2.0, 1024), (84.0, 2.0, 2048), (84.0, 2.0, 4096),
-                                            (6.0, 0.5, 1024)])
+                                            (6.0, 0.5, 1024), (200.0, 2.0, 8192)])
 def test_taps_match_oracle_quadrature(torch, fd, orc, zmax, dz, seglen):
     with fd.Plan(1 << 14, zmax, dz, seglen, 0) as plan:
         plan.make_templates()
@@ -86,7 +86,8 @@ def test_taps_match_oracle_quadrature(torch, fd, orc, zmax, dz, seglen):
             assert np.max(np.abs(got - ref)) < 1e-12, (k, z)
 
 
-@pytest.mark.parametrize("zmax,dz,seglen", [(20.0, 2.0, 1024), (84.0, 2.0, 2048), (84.0, 2.0, 4096)])
+@pytest.mark.parametrize("zmax,dz,seglen", [(20.0, 2.0, 1024), (84.0, 2.0, 2048), (84.0, 2.0, 4096),
+                                            (200.0, 2.0, 8192), (20.0, 2.0, 8192)])
 def test_template_spectra_match_fp64_fft_of_oracle_taps(torch, fd, orc, zmax, dz, seglen):
     with fd.Plan(1 << 14, zmax, dz, seglen, 0) as plan:
         plan.make_templates()
@@ -115,7 +116,8 @@ def test_config1_full_plane(torch, fd, orc, syn):
     assert np.max(np.abs(plane[10] - (a.real ** 2 + a.imag ** 2))) < 2e-5 * np.max(plane[10])
 
 
-@pytest.mark.parametrize("cfg,nbins", [(1, 1 << 18), (1, 100003), (2, 1 << 17), (4, 1 << 17), (2, 77777)])
+@pytest.mark.parametrize("cfg,nbins", [(1, 1 << 18), (1, 100003), (2, 1 << 17), (4, 1 << 17), (2, 77777),
+                                       (3, 1 << 17), (3, 55555)])
 def test_reduced_configs_full_plane(torch, fd, orc, syn, cfg, nbins):
     c = syn.CONFIGS[cfg]
     spec, _ = syn.config_spectrum(cfg, 0, nbins)
@@ -156,6 +158,33 @@ def test_config3_full_size_sampled_rows(torch, fd, orc, syn):
                                [0, 1, plane.shape[1] - 2, plane.shape[1] - 1]])
         ref = orc.plane_cells(spec, z, cols, True)
         assert np.max(np.abs(plane[k, cols] - ref)) <= TOL_MAX * np.max(plane[k])
+
+
+def test_config4_full_size_sampled_rows(torch, fd, orc, syn):
+    c = syn.CONFIGS[3]                                   # 201 templates, seglen 8192 (2 x 4096 kernel)
+    spec = syn.noise_only_c64(c["nbins"], 4242)
+    spec[7654321] += 30.0
+    plane, info = run_gpu(torch, fd, spec, c["zmax"], c["dz"], c["seglen"], 0)
+    assert plane.shape == (201, 1 << 23)
+    assert info["seglen"] == 8192 and info["useful"] + 2 * info["overlap"] == 8192
+    assert np.all(np.isfinite(plane))
+    check_rows(orc, spec, plane, c["zmax"], c["dz"], 0, rows=[0, 57, 100, 200])
+    rng = np.random.default_rng(6)
+    zs = orc.bank_z(c["zmax"], c["dz"])
+    B = info["useful"]
+    seams = np.array([B - 1, B, B + 1, 2 * B - 1, 2 * B, 500 * B - 1, 500 * B])   # segment boundaries
+    for k, z in enumerate(zs):
+        cols = np.concatenate([rng.integers(0, plane.shape[1], 2000), seams,
+                               [0, 1, plane.shape[1] - 2, plane.shape[1] - 1]])
+        ref = orc.plane_cells(spec, z, cols, False)
+        assert np.max(np.abs(plane[k, cols] - ref)) <= TOL_MAX * np.max(plane[k])
+
+
+@pytest.mark.parametrize("nbins", [1, 100, 7935, 7936, 7937, 20001])
+def test_seglen_8192_tiny_and_ragged(torch, fd, orc, syn, nbins):
+    spec = syn.make_spectrum(nbins, 800 + nbins, [(nbins / 2.0, -30.0, 10.0)] if nbins > 200 else [])
+    plane, info = run_gpu(torch, fd, spec, 40.0, 4.0, 8192, 0)
+    check_rows(orc, spec, plane, 40.0, 4.0, 0)
 
 
 def test_config5_batch_on_one_stream(torch, fd, orc, syn):
@@ -218,6 +247,8 @@ def test_segmentation_independence_on_gpu(torch, fd, syn):
     a, _ = run_gpu(torch, fd, spec, 20.0, 2.0, 1024, 0)
     b, _ = run_gpu(torch, fd, spec, 20.0, 2.0, 4096, 0)
     assert np.max(np.abs(a - b)) < 2e-5 * np.max(a)
+    c, _ = run_gpu(torch, fd, spec, 20.0, 2.0, 8192, 0)
+    assert np.max(np.abs(a - c)) < 2e-5 * np.max(a)
 
 
 def test_error_codes_on_device(torch, fd):

@@ -333,14 +333,16 @@ __device__ __forceinline__ void flush_edges(const KernelParams &prm, const Threa
     const float4 b = (tm.warp < G::W - 1) ? eb[(G::W + tm.warp + 1) * 16 + n1]  // y[n+1]: next warp's lane 0
                                           : eb[G::W * 16 + min(n1 + 1, 15)];    // ... or thread 0's next n1
     const bool lo = tm.lane < 16;                                             // lanes 0-15: p row, 16-31: q row
-    const float dr = lo ? a.x - b.x : a.y - b.y;
-    const float di = lo ? a.z - b.z : a.w - b.w;
+    const float ar = lo ? a.x : a.y, ai = lo ? a.z : a.w;
+    const float dr = ar - (lo ? b.x : b.y);
+    const float di = ai - (lo ? b.z : b.w);
+    const float pw = fmaf(ai, ai, ar * ar);
     const float ph = IB * fmaf(di, di, dr * dr);
     const int n = n1 * G::Q + 32 * tm.warp + 31;
     const long long col = pd.col0 + n;
     const int row = lo ? pd.pair : prm.ntemplates - 1 - pd.pair;
-    if (n >= prm.overlap && n < prm.overlap + prm.useful && col < prm.nbins)
-        st_stream(prm.plane + (size_t)row * prm.ncols + 2 * col + 1, ph);
+    st_stream2_if(prm.plane + (size_t)row * prm.ncols + 2 * col, pw, ph,
+                  n >= prm.overlap && n < prm.overlap + prm.useful && col < prm.nbins);
     pd.on = false;
 }
 
@@ -455,20 +457,17 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
                 st_stream_if(bq + n1 * G::Q, pw.y, vm & (1u << n1));
             }
         } else {
-            float4 *eb = edges + par * (2 * G::W * 16);
-            if (tm.lane == 31) {
+            // lanes 0 and 31 post their y to the mailbox; lane 31's cells (power and half-bin) are
+            // written one unit later by flush_edges, every other lane stores (P[n], P[n+1/2]) now
+            float4 *eb = edges + par * (2 * G::W * 16) + (tm.lane == 0 ? G::W * 16 : 0) + tm.warp * 16;
+            if (tm.lane == 31 || tm.lane == 0) {
 #pragma unroll
                 for (int n1 = 0; n1 < 16; ++n1)
-                    eb[tm.warp * 16 + n1] = make_float4(y[n1].re.x, y[n1].re.y, y[n1].im.x, y[n1].im.y);
-            }
-            if (tm.lane == 0) {
-#pragma unroll
-                for (int n1 = 0; n1 < 16; ++n1)
-                    eb[(G::W + tm.warp) * 16 + n1] = make_float4(y[n1].re.x, y[n1].re.y, y[n1].im.x, y[n1].im.y);
+                    eb[n1] = make_float4(y[n1].re.x, y[n1].re.y, y[n1].im.x, y[n1].im.y);
             }
             float *bp = prm.plane + (size_t)row_p * prm.ncols + 2 * (col0 + tid);
             float *bq = prm.plane + (size_t)row_q * prm.ncols + 2 * (col0 + tid);
-            const unsigned last = tm.lane == 31;
+            if (tm.lane == 31) vm = 0;
 #pragma unroll
             for (int n1 = 0; n1 < 16; ++n1) {
                 cpk d;                                   // y[n] - y[n+1], neighbour from lane + 1
@@ -478,11 +477,8 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
                                                   __shfl_down_sync(0xffffffffu, y[n1].im.y, 1)));
                 const float2 pw = power2(y[n1]);
                 const float2 ph = mul2(power2(d), bc2(IB));
-                const unsigned v = (vm >> n1) & 1u;
-                st_stream2_if(bp + 2 * n1 * G::Q, pw.x, ph.x, v & ~last);
-                st_stream2_if(bq + 2 * n1 * G::Q, pw.y, ph.y, v & ~last);
-                st_stream_if(bp + 2 * n1 * G::Q, pw.x, v & last);   // half-bin follows in flush_edges
-                st_stream_if(bq + 2 * n1 * G::Q, pw.y, v & last);
+                st_stream2_if(bp + 2 * n1 * G::Q, pw.x, ph.x, vm & (1u << n1));
+                st_stream2_if(bq + 2 * n1 * G::Q, pw.y, ph.y, vm & (1u << n1));
             }
             pend.col0 = col0;
             pend.pair = pair;

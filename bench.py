@@ -38,6 +38,11 @@ def load_peaks():
     return {"hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)"}
 
 
+# DRAM bytes (read + write) per launch of the fused kernel, from `ncu --set full` (dram__bytes_read.sum +
+# dram__bytes_write.sum): profiles/r1c_ncu_config{2,3,4,5}.md.  None where no capture exists.
+NCU_TRAFFIC_BYTES = {2: 671.6e6, 3: 5772.5e6, 4: 7575.0e6, 5: 1395.6e6}
+
+
 def workload(cfg_idx: int):
     from paper_1804_05335_b200 import synthetic
     c = dict(synthetic.CONFIGS[cfg_idx - 1])
@@ -278,14 +283,17 @@ def main():
         t_alu = w["alg_flops"] / (fp32_peak * 1e12)
         ach_gbs = w["alg_bytes"] / avg_kernel_s / 1e9
         ach_tf = w["alg_flops"] / avg_kernel_s / 1e12
+        traffic = NCU_TRAFFIC_BYTES.get(args.config)
         hbm = {"bound": "hbm", "achieved": ach_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-               "frac": ach_gbs / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"]}
+               "frac": ach_gbs / peaks["hbm_gbs"], "traffic": traffic, "peak_source": peaks["source"]}
         alu = {"bound": "alu", "achieved": ach_tf, "peak": fp32_peak, "unit": "TFLOP/s",
-               "frac": ach_tf / fp32_peak, "traffic": None,
+               "frac": ach_tf / fp32_peak, "traffic": traffic,
                "peak_source": f"{info.sm_count} SMs x 128 FP32 lanes x 2 x {sm_max_mhz:.0f} MHz (DESIGN.md)",
                "fma_probe_tflops": fp32_probe}
         roof = dict(alu if t_alu >= t_hbm else hbm)      # north_star: the slower bound is the roofline
-        roof.update(kernel="fdas_fused_kernel", kernel_ms=avg_kernel_s * 1e3,
+        roof.update(kernel="fdas_fused_kernel_8k" if w["seglen"] == 8192 else "fdas_fused_kernel",
+                    traffic_source="ncu --set full, profiles/r1c_ncu_config%d.md (bytes per launch)" % args.config
+                    if traffic else None, kernel_ms=avg_kernel_s * 1e3,
                     alg_bytes=w["alg_bytes"], alg_flops=w["alg_flops"],
                     t_bound_ms={"hbm": t_hbm * 1e3, "alu": t_alu * 1e3},
                     hbm=hbm if roof["bound"] == "alu" else None, alu=alu if roof["bound"] == "hbm" else None)

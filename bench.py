@@ -188,6 +188,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--probe", action="store_true",
+                    help="print the instruction-cost probes (fdas_probe_pipes) as one JSON line and exit")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -199,6 +201,18 @@ def main():
     import numpy as np
     import torch
     from paper_1804_05335_b200 import dist, fdas, synthetic
+
+    if args.probe:
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py --probe needs a CUDA device")
+        torch.cuda.set_device(0)
+        pr = fdas.fdas_probe_pipes(None, 2000)
+        print(json.dumps({"probe": "cycles per warp instruction (fdas_probe_pipes, include/fdas.h)",
+                          "per_sm_subpartition": {k: pr[k] for k in ("ffma", "fadd2", "ffma2_bcast", "ffma2_3pair", "fmul2")},
+                          "per_sm": {k: pr[k] for k in ("lds_sts64", "shfl")},
+                          "mix_round_cycles_per_sm": pr["mix_round"],
+                          "fp32_fma_probe_tflops": fdas.fdas_measure_fp32_peak(None, 4000)}))
+        return
 
     rank, local_rank, world = dist.init()
     if not torch.cuda.is_available():

@@ -136,6 +136,18 @@ fdas_status fdas_get_template_spectrum(fdas_plan *plan, int32_t k, float *host_r
  */
 fdas_status fdas_measure_fp32_peak(void *stream, int32_t iters, double *tflops);
 
+/*
+ * Instruction-cost probes: cycles per warp instruction measured with
+ * clock64 on one CTA of 8 warps per SM, `iters` rounds each.  out[0..7] (nout >= 8):
+ *   [0] scalar FFMA, [1] FADD2, [2] FFMA2 (pair * broadcast scalar + pair), [3] FFMA2 with three
+ *   distinct register pairs, [4] FMUL2            -- per SM sub-partition (2 warps each);
+ *   [5] conflict-free LDS.64 / STS.64, [6] SHFL  -- per SM (8 warps share the load/store pipe);
+ *   [7] cycles per SM for one round of the unit-shaped mix: per warp 16 LDS.64 + 16 STS.64 +
+ *       128 packed FP32 instructions, 8 warps.
+ * Synchronises `stream`.
+ */
+fdas_status fdas_probe_pipes(void *stream, int32_t iters, double *out, int32_t nout);
+
 /* Number of kernels the library has launched in this process (for bench accounting). */
 int64_t fdas_launch_count(void);
 

@@ -3,6 +3,7 @@
 // of fdas_templates.cuh / fdas_kernel.cuh; there is no CPU fallback.
 #include "../../include/fdas.h"
 #include "fdas_templates.cuh"
+#include "fdas_probe.cuh"
 
 #include <atomic>
 #include <cmath>
@@ -363,3 +364,48 @@ fdas_status fdas_measure_fp32_peak(void *stream, int32_t iters, double *tflops)
 }
 
 } // extern "C"
+
+namespace {
+template <int MODE>
+cudaError_t run_probe(cudaStream_t st, float *d_out, int sms, int iters, double *cycles_per_instr)
+{
+    const int threads = 256;                       // 8 warps: two per SM sub-partition
+    const size_t smem = (size_t)16 * threads * sizeof(float2);
+    probe_kernel<MODE><<<sms, threads, smem, st>>>(d_out, 8, 1.0001f, 0.9999f);        // warm-up
+    probe_kernel<MODE><<<sms, threads, smem, st>>>(d_out, iters, 1.0001f, 0.9999f);
+    g_launches += 2;
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return e;
+    float h[2];
+    e = cudaMemcpy(h, d_out, sizeof(h), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return e;
+    const bool per_sm = (MODE == PROBE_LDS_STS64 || MODE == PROBE_SHFL || MODE == PROBE_MIX);
+    // FP modes: per SM sub-partition (2 warps each); memory modes: per SM (8 warps share one LSU)
+    const double warps = (MODE == PROBE_MIX) ? 1.0 : per_sm ? 8.0 : 2.0;   // mix: whole round of the CTA
+    *cycles_per_instr = (double)h[1] / ((double)iters * probe_instr_per_round(MODE) * warps);
+    return cudaGetLastError();
+}
+} // namespace
+
+extern "C" fdas_status fdas_probe_pipes(void *stream, int32_t iters, double *out, int32_t nout)
+{
+    if (!out || iters <= 0 || nout < (int)PROBE_COUNT) return FDAS_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    float *d_out = nullptr;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaMalloc(&d_out, 64) != cudaSuccess)
+        return FDAS_ERR_CUDA;
+    cudaError_t e = cudaSuccess;
+    if (e == cudaSuccess) e = run_probe<PROBE_FFMA>(st, d_out, sms, iters, &out[PROBE_FFMA]);
+    if (e == cudaSuccess) e = run_probe<PROBE_FADD2>(st, d_out, sms, iters, &out[PROBE_FADD2]);
+    if (e == cudaSuccess) e = run_probe<PROBE_FFMA2>(st, d_out, sms, iters, &out[PROBE_FFMA2]);
+    if (e == cudaSuccess) e = run_probe<PROBE_FFMA2_3PAIR>(st, d_out, sms, iters, &out[PROBE_FFMA2_3PAIR]);
+    if (e == cudaSuccess) e = run_probe<PROBE_FMUL2>(st, d_out, sms, iters, &out[PROBE_FMUL2]);
+    if (e == cudaSuccess) e = run_probe<PROBE_LDS_STS64>(st, d_out, sms, iters, &out[PROBE_LDS_STS64]);
+    if (e == cudaSuccess) e = run_probe<PROBE_SHFL>(st, d_out, sms, iters, &out[PROBE_SHFL]);
+    if (e == cudaSuccess) e = run_probe<PROBE_MIX>(st, d_out, sms, iters, &out[PROBE_MIX]);
+    cudaFree(d_out);
+    return e == cudaSuccess ? FDAS_OK : FDAS_ERR_CUDA;
+}

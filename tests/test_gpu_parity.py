@@ -241,6 +241,17 @@ def test_deterministic_and_linear(torch, fd, syn):
     assert np.array_equal(p4, 4.0 * p1)                  # power-of-two scaling is exact in fp32
 
 
+@pytest.mark.parametrize("seglen,interbin", [(2048, 0), (2048, 1), (4096, 1), (8192, 0)])
+def test_bitwise_repeatable_all_kernels(torch, fd, syn, seglen, interbin):
+    # compute-sanitizer is closed on this pool; a race in the shared-memory exchange pipeline
+    # (split-phase mbarriers, per-warp regions, mailbox) would show up as run-to-run differences
+    spec = syn.make_spectrum(300000, 75, [(150000.3, 6.0, 20.0)])
+    ref, _ = run_gpu(torch, fd, spec, 20.0, 2.0, seglen, interbin)
+    for _ in range(4):
+        again, _ = run_gpu(torch, fd, spec, 20.0, 2.0, seglen, interbin)
+        assert np.array_equal(ref, again)
+
+
 def test_segmentation_independence_on_gpu(torch, fd, syn):
     # P10 on the device: the plane does not depend on the segment length
     spec = syn.make_spectrum(50000, 74, [(25000.0, -6.0, 12.0)])

@@ -12,6 +12,7 @@
 #pragma once
 #include "fdas_kernel.cuh"
 #include "fdas_kernel8k.cuh"
+#include "fdas_kernel2.cuh"
 
 namespace fdas {
 

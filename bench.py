@@ -39,8 +39,9 @@ def load_peaks():
 
 
 # DRAM bytes (read + write) per launch of the fused kernel, from `ncu --set full` (dram__bytes_read.sum +
-# dram__bytes_write.sum): profiles/r1c_ncu_config{2,3,4,5}.md.  None where no capture exists.
-NCU_TRAFFIC_BYTES = {2: 671.6e6, 3: 5772.5e6, 4: 7575.0e6, 5: 1395.6e6}
+# dram__bytes_write.sum): profiles/r1c_ncu_config{2,4,5}.md, profiles/r1d_ncu_config3.md.  None where no capture exists.
+NCU_TRAFFIC_BYTES = {2: 671.6e6, 3: 5752.6e6, 4: 7575.0e6, 5: 1395.6e6}
+NCU_TRAFFIC_FILE = {2: "r1c_ncu_config2.md", 3: "r1d_ncu_config3.md", 4: "r1c_ncu_config4.md", 5: "r1c_ncu_config5.md"}
 
 
 def workload(cfg_idx: int):
@@ -305,8 +306,8 @@ def main():
                "peak_source": f"{info.sm_count} SMs x 128 FP32 lanes x 2 x {sm_max_mhz:.0f} MHz (DESIGN.md)",
                "fma_probe_tflops": fp32_probe}
         roof = dict(alu if t_alu >= t_hbm else hbm)      # north_star: the slower bound is the roofline
-        roof.update(kernel="fdas_fused_kernel_8k" if w["seglen"] == 8192 else "fdas_fused_kernel",
-                    traffic_source="ncu --set full, profiles/r1c_ncu_config%d.md (bytes per launch)" % args.config
+        roof.update(kernel={8192: "fdas_fused_kernel_8k", 4096: "fdas_fused_kernel2"}.get(w["seglen"], "fdas_fused_kernel"),
+                    traffic_source="ncu --set full, profiles/%s (bytes per launch)" % NCU_TRAFFIC_FILE[args.config]
                     if traffic else None, kernel_ms=avg_kernel_s * 1e3,
                     alg_bytes=w["alg_bytes"], alg_flops=w["alg_flops"],
                     t_bound_ms={"hbm": t_hbm * 1e3, "alu": t_alu * 1e3},

@@ -103,26 +103,15 @@ __device__ __forceinline__ void rotate_xhat(const float2 *__restrict__ wtab, con
         }
 }
 
-// Q3 (products, inverse DFT_R3, twiddle), the shuffle exchange, and Q2's DFT16 + twiddle.
-// Returns the 16 values this thread stores to E1 (index n2).
+// Tail of Q3 (inverse DFT_R3, twiddle), the shuffle exchange, and Q2's DFT16 + twiddle, starting
+// from the products a[j][k3].  Returns the 16 values this thread stores to E1 (index n2).
 template <int L>
-__device__ __forceinline__ void inv_q3_q2(const float2 (&xh)[Geo<L>::PTS], const float4 (&h4)[Geo<L>::PTS / 2],
-                                          const InvTwiddles2<L> &tw, const ThreadMap<L> &tm, cpk (&out)[16])
+__device__ __forceinline__ void q3_tail_q2(cpk (&a)[Geo<L>::NB3][Geo<L>::R3], const InvTwiddles2<L> &tw,
+                                           const ThreadMap<L> &tm, cpk (&out)[16])
 {
     using G = Geo<L>;
-    cpk a[G::NB3][G::R3];
 #pragma unroll
     for (int j = 0; j < G::NB3; ++j) {
-#pragma unroll
-        for (int k3 = 0; k3 < G::R3; ++k3) {
-            const int i = j * G::R3 + k3;
-            const float4 hh = h4[i >> 1];
-            const float2 h = (i & 1) ? make_float2(hh.z, hh.w) : make_float2(hh.x, hh.y);
-            const float2 x = xh[i];
-            const float ac = x.x * h.x, bc = x.y * h.x;
-            a[j][k3].re = make_float2(fmaf(-x.y, h.y, ac), fmaf(x.y, h.y, ac));
-            a[j][k3].im = make_float2(fmaf(x.x, h.y, bc), fmaf(-x.x, h.y, bc));
-        }
         dft<+1, G::R3>(a[j]);
 #pragma unroll
         for (int r = 0; r < G::R3; ++r) a[j][r] = cmul(a[j][r], tw.tw3r[j][r]);
@@ -176,6 +165,29 @@ __device__ __forceinline__ void inv_q3_q2(const float2 (&xh)[Geo<L>::PTS], const
             out[2 * nh + 1] = cmul(u1[nh], tw.tw2p[2 * nh + 1]);
         }
     }
+}
+
+// Q3 products p = X^ H, q = X^ conj(H), then q3_tail_q2.
+template <int L>
+__device__ __forceinline__ void inv_q3_q2(const float2 (&xh)[Geo<L>::PTS], const float4 (&h4)[Geo<L>::PTS / 2],
+                                          const InvTwiddles2<L> &tw, const ThreadMap<L> &tm, cpk (&out)[16])
+{
+    using G = Geo<L>;
+    cpk a[G::NB3][G::R3];
+#pragma unroll
+    for (int j = 0; j < G::NB3; ++j) {
+#pragma unroll
+        for (int k3 = 0; k3 < G::R3; ++k3) {
+            const int i = j * G::R3 + k3;
+            const float4 hh = h4[i >> 1];
+            const float2 h = (i & 1) ? make_float2(hh.z, hh.w) : make_float2(hh.x, hh.y);
+            const float2 x = xh[i];
+            const float ac = x.x * h.x, bc = x.y * h.x;
+            a[j][k3].re = make_float2(fmaf(-x.y, h.y, ac), fmaf(x.y, h.y, ac));
+            a[j][k3].im = make_float2(fmaf(x.x, h.y, bc), fmaf(-x.x, h.y, bc));
+        }
+    }
+    q3_tail_q2<L>(a, tw, tm, out);
 }
 
 template <int L, bool INTERBIN, int MINB>
@@ -340,6 +352,8 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
         if (pend[1].on) flush_edges<L>(prm, tm, edges, pend[1]);
     }
 }
+
+
 
 #endif // __CUDACC__
 

@@ -141,6 +141,70 @@ def cpu_baseline(w, budget_s=15.0):
                       f"{w['nbins']} bins of {w['name']}, fp64 direct correlation, {dt:.1f} s"}
 
 
+class CufftUnfused:
+    """
+    Same-box comparator: the paper's variant A restated with
+    library FFTs -- overlapped segments copied out, cuFFT forward (torch.fft), a broadcast multiply by every
+    template spectrum, cuFFT inverse, then discard + power (+ interbin), each step a global-memory round trip.
+    Harness-side only: it is what the fused kernel is compared WITH (the paper's headline ratio is
+    "custom vs cuFFT"), never part of the product path.  Segmentation (overlap, useful points)
+    and the taps come from the plan so both sides compute the same function.
+    """
+
+    def __init__(self, torch, plan, dev):
+        import numpy as np
+        from paper_1804_05335_b200 import fdas
+        self.torch = torch
+        info = plan.info
+        self.N, self.K, self.L = int(info.nbins), int(info.ntemplates), int(info.seglen)
+        self.ov, self.B, self.nseg = int(info.overlap), int(info.useful), int(info.nseg)
+        self.interbin = bool(info.interbin)
+        g = np.zeros((self.K, self.L), dtype=np.complex128)
+        for k in range(self.K):
+            h = fdas.fdas_get_taps(plan.handle, k)           # h[d + m_k], d = -m_k..m_k
+            mk = (h.size - 1) // 2
+            d = np.arange(-mk, mk + 1)
+            g[k, (-d) % self.L] = np.conj(h)                  # correlation as circular convolution
+        self.H = torch.from_numpy((np.fft.fft(g, axis=1) / self.L).astype(np.complex64)).to(dev)
+        self.padded = torch.zeros(self.ov + self.nseg * self.B + self.L, dtype=torch.complex64, device=dev)
+
+    def run(self, d_spec, d_plane):
+        torch = self.torch
+        N, K, L, ov, B, nseg = self.N, self.K, self.L, self.ov, self.B, self.nseg
+        self.padded[ov:ov + N] = torch.view_as_complex(d_spec)                # zero extension both sides (R7)
+        segs = self.padded.unfold(0, L, B)[:nseg].contiguous()               # step 1: overlapped segments
+        X = torch.fft.fft(segs, dim=1)                                       # step 2: cuFFT forward
+        Y = X.unsqueeze(0) * self.H.unsqueeze(1)                             # step 3: K x nseg x L products
+        y = torch.fft.ifft(Y, dim=2, norm="forward")                         # step 4: cuFFT inverse (1/L in H)
+        del Y
+        if not self.interbin:                                                # step 5: discard + power
+            yv = torch.view_as_real(y[:, :, ov:ov + B])
+            P = (yv[..., 0] ** 2 + yv[..., 1] ** 2).reshape(K, nseg * B)
+            d_plane.copy_(P[:, :N])
+        else:
+            yv = y[:, :, ov:ov + B + 1]
+            a = torch.view_as_real(yv[:, :, :B])
+            dd = torch.view_as_real(yv[:, :, :B] - yv[:, :, 1:])
+            out = torch.empty((K, nseg * B, 2), dtype=torch.float32, device=d_plane.device)
+            out[:, :, 0] = (a[..., 0] ** 2 + a[..., 1] ** 2).reshape(K, nseg * B)
+            out[:, :, 1] = ((math.pi / 4) ** 2 * (dd[..., 0] ** 2 + dd[..., 1] ** 2)).reshape(K, nseg * B)
+            d_plane.copy_(out[:, :N].reshape(K, 2 * N))
+
+
+def time_cufft(torch, plan, dev, d_spec, d_plane, steps=5, warmup=2):
+    cmp_ = CufftUnfused(torch, plan, dev)
+    for _ in range(warmup):
+        cmp_.run(d_spec, d_plane)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        cmp_.run(d_spec, d_plane)
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / steps
+
+
 def run_reference(args, w):
     """--impl reference: the oracle timed on the host cores (rank 0 only)."""
     rank = int(os.environ.get("RANK", "0"))
@@ -189,6 +253,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cufft", action="store_true",
+                    help="skip the same-box unfused cuFFT comparator (variant A of the paper, N = 1 only)")
     ap.add_argument("--probe", action="store_true",
                     help="print the instruction-cost probes (fdas_probe_pipes) as one JSON line and exit")
     args = ap.parse_args()
@@ -290,6 +356,12 @@ def main():
 
     fp32_probe = fdas.fdas_measure_fp32_peak(stream, 4000) if rank == 0 else None
 
+    # ---- same-box comparator: the paper's unfused cuFFT pipeline (harness-side, N = 1 only)
+    cufft_ms = None
+    if world == 1 and not args.no_cufft:
+        del h_out
+        cufft_ms = time_cufft(torch, plan, dev, d_in[0], d_out[0])
+
     if rank == 0:
         avg_kernel_s = (sum(kern_ms) / len(kern_ms)) * 1e-3
         sm_max_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
@@ -331,6 +403,12 @@ def main():
             "clocks": clocks,
             "roofline": roof,
         }
+        if cufft_ms is not None:
+            out["cufft_unfused"] = {"ms_per_step": cufft_ms, "value": w["cells"] / (cufft_ms * 1e-3), "unit": UNIT,
+                                    "fused_speedup": cufft_ms / (avg_kernel_s * 1e3),
+                                    "what": "paper's variant A on this GPU (PAPER.md:101-119): segment copy, torch.fft "
+                                            "(cuFFT) forward, broadcast multiply, cuFFT inverse, discard + power; "
+                                            "context for the paper's custom-vs-cuFFT ratio (PAPER.md:237), not a target"}
         if not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(w)
         print(json.dumps(out))

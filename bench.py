@@ -357,10 +357,13 @@ def main():
     fp32_probe = fdas.fdas_measure_fp32_peak(stream, 4000) if rank == 0 else None
 
     # ---- same-box comparator: the paper's unfused cuFFT pipeline (harness-side, N = 1 only)
-    cufft_ms = None
+    cufft_ms, cufft_err = None, None
     if world == 1 and not args.no_cufft:
         del h_out
-        cufft_ms = time_cufft(torch, plan, dev, d_in[0], d_out[0])
+        try:
+            cufft_ms = time_cufft(torch, plan, dev, d_in[0], d_out[0])
+        except Exception as exc:                      # a comparator failure must not cost the bench line
+            cufft_err = f"{type(exc).__name__}: {exc}"[:200]
 
     if rank == 0:
         avg_kernel_s = (sum(kern_ms) / len(kern_ms)) * 1e-3
@@ -409,6 +412,8 @@ def main():
                                     "what": "paper's variant A on this GPU (PAPER.md:101-119): segment copy, torch.fft "
                                             "(cuFFT) forward, broadcast multiply, cuFFT inverse, discard + power; "
                                             "context for the paper's custom-vs-cuFFT ratio (PAPER.md:237), not a target"}
+        elif cufft_err:
+            out["cufft_unfused"] = {"unavailable": cufft_err}
         if not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(w)
         print(json.dumps(out))

@@ -21,7 +21,9 @@ Pins (tests/test_oracle_pins.py): closed form via scipy's Fresnel integrals, the
 sinc/delta special case, brute-force time-domain chirp + DFT, injected-chirp peak,
 reversal / shift / linearity invariants, noise statistics, the paper's printed
 interbinning losses, fp64 FFT overlap-save at two segment lengths,
-and a pure-Python triple loop on tiny inputs.  No function here is "parity unpinned".
+and a pure-Python triple loop on tiny inputs; the threshold search (`candidates`) by the
+exponential tail law of noise powers, the 0 / +inf thresholds and an injected chirp's cell.
+No function here is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -226,6 +228,24 @@ def plane_cells(spectrum, z: float, cols, interbin: bool = False) -> np.ndarray:
     odd = (cols % 2) == 1
     return np.where(odd, power_from_amplitudes(INTERBIN_SCALE * (y0 - y1)),
                     power_from_amplitudes(y0))
+
+
+def candidates(spectrum, zmax: float, dz: float, threshold: float, interbin: bool = False):
+    """
+    Threshold search of the plane ("calculating the power spectrum, and comparing the
+    resulting Fourier power to a pre-calculated threshold"; PAPER.md:331 names search / candidate
+    selection next to the correlation as the step to fuse; reading R15): every cell with
+    P[k][c] > threshold (strict), as three arrays (row k, column c, power) sorted by (row, column).
+    Row by row, so the plane is never held.
+    """
+    rows, cols, pows = [], [], []
+    for k, z in enumerate(bank_z(zmax, dz)):
+        p = plane_row(spectrum, z, interbin)
+        c = np.nonzero(p > threshold)[0]
+        rows.append(np.full(c.size, k, dtype=np.int64))
+        cols.append(c.astype(np.int64))
+        pows.append(p[c])
+    return np.concatenate(rows), np.concatenate(cols), np.concatenate(pows)
 
 
 def cmacs(n: int, zmax: float, dz: float) -> int:

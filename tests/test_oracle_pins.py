@@ -281,3 +281,53 @@ def test_p10_overlap_save_equals_direct(seglen):
 def test_cmacs_count():
     # 6.0e7 complex MACs for config 1
     assert orc.cmacs(1 << 16, 20.0, 2.0) == (1 << 16) * 913
+
+
+# ---------------------------------------------------------------- P11: threshold search (reading R15)
+def test_p11_threshold_limits_and_z0_row():
+    a = syn.make_spectrum(1 << 14, 61)
+    n = a.size
+    for ib in (False, True):
+        ncols = 2 * n if ib else n
+        rows, cols, pows = orc.candidates(a, 4.0, 2.0, -1.0, ib)          # below every power: every cell
+        assert rows.size == 5 * ncols and np.array_equal(cols[:ncols], np.arange(ncols))
+        rows, cols, pows = orc.candidates(a, 4.0, 2.0, float("inf"), ib)  # above every power: nothing
+        assert rows.size == 0
+    # z = 0 row: h_0 is the Kronecker delta (P2), so its candidates are the raw bins with |A|^2 > thr
+    rows, cols, pows = orc.candidates(a, 4.0, 2.0, 5.0)
+    raw = np.abs(a.astype(np.complex128)) ** 2
+    assert np.array_equal(cols[rows == 2], np.nonzero(raw > 5.0)[0])
+    assert np.array_equal(pows[rows == 2], raw[raw > 5.0])
+    # sorted by (row, col), strict inequality
+    key = rows * (1 << 40) + cols
+    assert np.all(np.diff(key) > 0) and np.all(pows > 5.0)
+
+
+def test_p11_noise_tail_law():
+    # unit-power white noise -> filtered powers are exponential with mean E_z = sum|h_z|^2 (P8), so the
+    # expected count above thr in row z is N exp(-thr / E_z)
+    a = syn.make_spectrum(1 << 17, 62)
+    thr = 6.0
+    rows, cols, pows = orc.candidates(a, 20.0, 10.0, thr)
+    for k, z in enumerate(orc.bank_z(20.0, 10.0)):
+        e = np.sum(np.abs(orc.taps(z)) ** 2)
+        expect = a.size * math.exp(-thr / e)
+        got = int(np.sum(rows == k))
+        assert abs(got - expect) < 5.0 * math.sqrt(expect) * 1.5, (z, got, expect)   # neighbours correlate: loose
+
+
+def test_p11_injected_chirp_is_the_candidate():
+    n, r0, z0, amp = 1 << 13, 3000, 8.0, 50.0
+    a = syn.chirp_spectrum(n, [(float(r0), z0, amp)]).astype(np.complex64)
+    zs = orc.bank_z(20.0, 2.0)
+    k0 = int(np.nonzero(zs == z0)[0][0])
+    rows, cols, pows = orc.candidates(a, 20.0, 2.0, 0.9 * amp ** 2)
+    assert rows.size >= 1
+    i = int(np.argmax(pows))
+    assert (rows[i], cols[i]) == (k0, r0) and abs(pows[i] - amp ** 2) < 0.01 * amp ** 2
+    assert np.all(np.abs(rows - k0) <= 1) and np.all(np.abs(cols - r0) <= 1)
+    # half-bin tone, interbinned: the candidate sits in the odd column 2 r0 + 1 (P9 layout)
+    b = syn.chirp_spectrum(n, [(r0 + 0.5, 0.0, amp)]).astype(np.complex64)
+    rows, cols, pows = orc.candidates(b, 4.0, 2.0, 0.9 * amp ** 2, True)
+    i = int(np.argmax(pows))
+    assert (rows[i], cols[i]) == (2, 2 * r0 + 1)

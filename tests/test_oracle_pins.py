@@ -297,7 +297,7 @@ def test_p11_threshold_limits_and_z0_row():
     rows, cols, pows = orc.candidates(a, 4.0, 2.0, 5.0)
     raw = np.abs(a.astype(np.complex128)) ** 2
     assert np.array_equal(cols[rows == 2], np.nonzero(raw > 5.0)[0])
-    assert np.array_equal(pows[rows == 2], raw[raw > 5.0])
+    assert np.allclose(pows[rows == 2], raw[raw > 5.0], rtol=1e-14, atol=0)
     # sorted by (row, col), strict inequality
     key = rows * (1 << 40) + cols
     assert np.all(np.diff(key) > 0) and np.all(pows > 5.0)

@@ -109,6 +109,34 @@ fdas_status fdas_execute(fdas_plan *plan, void *stream, const void *d_spectrum, 
  */
 fdas_status fdas_execute_host(fdas_plan *plan, void *stream, const void *h_spectrum, float *h_plane);
 
+/*
+ * One cell of the plane above the threshold (16 bytes).
+ */
+typedef struct fdas_candidate {
+    int64_t col;    /* plane column (0..ncols-1; interbinned: 2r <-> bin r, 2r+1 <-> bin r + 1/2) */
+    int32_t row;    /* template row k <-> z_k = -zmax + k*dz                                       */
+    float power;    /* P[row][col], the value fdas_execute would have stored                       */
+} fdas_candidate;
+
+/*
+ * Threshold search fused behind the power step ("calculating the power spectrum,
+ * and comparing the resulting Fourier power to a pre-calculated threshold"; PAPER.md:331 names
+ * search / candidate selection on on-chip data as the step to fuse next; reading R15).
+ * Runs the same fused kernel as fdas_execute (steps a2-a7) but the plane is never written:
+ * every cell with P > threshold (strict; NaN never passes) is appended to `d_cands`.
+ *   d_spectrum : as for fdas_execute.
+ *   d_cands    : device, `capacity` entries, 16-byte aligned (may be NULL when capacity = 0).
+ *   d_count    : device, one uint64, 8-byte aligned; zeroed on `stream` by this call, then
+ *                incremented once per cell found.  *d_count may exceed `capacity`: only the
+ *                first min(*d_count, capacity) entries of d_cands are valid, in no defined
+ *                order (sort on (row, col) to compare), and WHICH cells were dropped when it
+ *                overflows is unspecified.
+ * Allocates nothing, never synchronises the host.  Errors as fdas_execute, plus
+ * FDAS_ERR_INVALID_ARG for a NaN threshold, capacity < 0 or a NULL d_count.
+ */
+fdas_status fdas_execute_threshold(fdas_plan *plan, void *stream, const void *d_spectrum, float threshold,
+                                   fdas_candidate *d_cands, int64_t capacity, uint64_t *d_count);
+
 /* Free the plan and everything it owns.  fdas_destroy(NULL) is a no-op returning FDAS_OK. */
 fdas_status fdas_destroy(fdas_plan *plan);
 

@@ -28,6 +28,7 @@ struct fdas_plan {
     float2 *d_stage_in;  // fdas_execute_host staging (lazy)
     float *d_stage_out;
     void (*kernel)(const KernelParams);
+    void (*kernel_thr)(const KernelParams);   // MODE 1: threshold search instead of the plane store
     char err[256];
 };
 
@@ -47,26 +48,30 @@ namespace {
 typedef void (*kernel_fn)(const KernelParams);
 
 template <int L, int MINB>
-kernel_fn pick_kernel(bool ib)
+kernel_fn pick_kernel(bool ib, int mode)
 {
+    if (mode) return ib ? (kernel_fn)fdas_fused_kernel<L, true, MINB, 1> : (kernel_fn)fdas_fused_kernel<L, false, MINB, 1>;
     return ib ? (kernel_fn)fdas_fused_kernel<L, true, MINB> : (kernel_fn)fdas_fused_kernel<L, false, MINB>;
 }
 
 // L = 4096: second-generation kernel (shuffle exchange, fdas_kernel2.cuh); measured on B200 it is
 // 4.5 % faster than the first at L = 4096 and 7 % slower at L = 2048, which stays on the first.
 template <int L, int MINB>
-kernel_fn pick_kernel2(bool ib)
+kernel_fn pick_kernel2(bool ib, int mode)
 {
+    if (mode) return ib ? (kernel_fn)fdas_fused_kernel2<L, true, MINB, 1> : (kernel_fn)fdas_fused_kernel2<L, false, MINB, 1>;
     return ib ? (kernel_fn)fdas_fused_kernel2<L, true, MINB> : (kernel_fn)fdas_fused_kernel2<L, false, MINB>;
 }
 
-kernel_fn select_kernel(int L, bool ib)
+// mode 0: plane store (fdas_execute); mode 1: threshold search (fdas_execute_threshold)
+kernel_fn select_kernel(int L, bool ib, int mode = 0)
 {
     switch (L) {
-    case 1024: return pick_kernel<1024, 4>(ib);
-    case 2048: return pick_kernel<2048, 2>(ib);
-    case 4096: return pick_kernel2<4096, 1>(ib);
-    case 8192: return ib ? nullptr : (kernel_fn)fdas_fused_kernel_8k<1>;   // 2 x 4096, no interbin
+    case 1024: return pick_kernel<1024, 4>(ib, mode);
+    case 2048: return pick_kernel<2048, 2>(ib, mode);
+    case 4096: return pick_kernel2<4096, 1>(ib, mode);
+    case 8192:                                                            // 2 x 4096, no interbin
+        return ib ? nullptr : mode ? (kernel_fn)fdas_fused_kernel_8k<1, 1> : (kernel_fn)fdas_fused_kernel_8k<1>;
     default: return nullptr;
     }
 }
@@ -139,6 +144,7 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double
     if (!p) return FDAS_ERR_NOMEM;
     std::memset(p, 0, sizeof(*p));
     p->kernel = kern;
+    p->kernel_thr = select_kernel(seglen, interbin != 0, 1);
     fdas_info &I = p->info;
     I.nbins = nbins;
     I.ncols = interbin ? 2 * nbins : nbins;
@@ -165,6 +171,8 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double
         if ((e = cudaGetDeviceProperties(&prop, p->device)) != cudaSuccess) { st = FDAS_ERR_CUDA; break; }
         I.sm_count = prop.multiProcessorCount;
         if ((e = cudaFuncSetAttribute((const void *)kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      I.smem_bytes)) != cudaSuccess) { st = FDAS_ERR_CUDA; break; }
+        if ((e = cudaFuncSetAttribute((const void *)p->kernel_thr, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       I.smem_bytes)) != cudaSuccess) { st = FDAS_ERR_CUDA; break; }
         cudaFuncAttributes fa;
         if ((e = cudaFuncGetAttributes(&fa, (const void *)kern)) != cudaSuccess) { st = FDAS_ERR_CUDA; break; }
@@ -228,15 +236,18 @@ fdas_status fdas_make_templates(fdas_plan *p, void *stream)
     return FDAS_OK;
 }
 
-fdas_status fdas_execute(fdas_plan *p, void *stream, const void *d_spectrum, float *d_plane)
+static fdas_status launch_fused(fdas_plan *p, void *stream, const void *d_spectrum, float *d_plane,
+                                float threshold, fdas_candidate *d_cands, int64_t capacity,
+                                unsigned long long *d_count)
 {
-    if (!p || !d_spectrum || !d_plane) return FDAS_ERR_INVALID_ARG;
-    if (!p->ready) return FDAS_ERR_NOT_READY;
-    if (((uintptr_t)d_spectrum & 15) || ((uintptr_t)d_plane & 15)) return FDAS_ERR_ALIGNMENT;
     const fdas_info &I = p->info;
     KernelParams prm;
     prm.spectrum = (const float2 *)d_spectrum;
     prm.plane = d_plane;
+    prm.cands = (Candidate *)d_cands;
+    prm.count = d_count;
+    prm.capacity = capacity;
+    prm.threshold = threshold;
     prm.hperm = (const float4 *)p->d_hperm;
     prm.wtab = p->d_wtab;
     prm.wtab2 = p->d_wtab2;
@@ -248,10 +259,32 @@ fdas_status fdas_execute(fdas_plan *p, void *stream, const void *d_spectrum, flo
     prm.overlap = I.overlap;
     prm.useful = I.useful;
     void *args[] = {&prm};
-    FDAS_CUDA(p, cudaLaunchKernel((const void *)p->kernel, dim3(I.grid), dim3(I.threads), args,
+    const void *kern = d_count ? (const void *)p->kernel_thr : (const void *)p->kernel;
+    FDAS_CUDA(p, cudaLaunchKernel(kern, dim3(I.grid), dim3(I.threads), args,
                                   (size_t)I.smem_bytes, (cudaStream_t)stream));
     g_launches += 1;
     return FDAS_OK;
+}
+
+fdas_status fdas_execute(fdas_plan *p, void *stream, const void *d_spectrum, float *d_plane)
+{
+    if (!p || !d_spectrum || !d_plane) return FDAS_ERR_INVALID_ARG;
+    if (!p->ready) return FDAS_ERR_NOT_READY;
+    if (((uintptr_t)d_spectrum & 15) || ((uintptr_t)d_plane & 15)) return FDAS_ERR_ALIGNMENT;
+    return launch_fused(p, stream, d_spectrum, d_plane, 0.f, nullptr, 0, nullptr);
+}
+
+fdas_status fdas_execute_threshold(fdas_plan *p, void *stream, const void *d_spectrum, float threshold,
+                                   fdas_candidate *d_cands, int64_t capacity, uint64_t *d_count)
+{
+    if (!p || !d_spectrum || !d_count || capacity < 0 || (capacity > 0 && !d_cands) || threshold != threshold)
+        return FDAS_ERR_INVALID_ARG;
+    if (!p->ready) return FDAS_ERR_NOT_READY;
+    if (((uintptr_t)d_spectrum & 15) || ((uintptr_t)d_cands & 15) || ((uintptr_t)d_count & 7))
+        return FDAS_ERR_ALIGNMENT;
+    FDAS_CUDA(p, cudaMemsetAsync(d_count, 0, sizeof(uint64_t), (cudaStream_t)stream));
+    return launch_fused(p, stream, d_spectrum, nullptr, threshold, d_cands, capacity,
+                        (unsigned long long *)d_count);
 }
 
 fdas_status fdas_execute_host(fdas_plan *p, void *stream, const void *h_spectrum, float *h_plane)

@@ -68,9 +68,20 @@ FDAS_HD void freq_to_reg(int f, int &tid, int &i)
     i = j * G::R3 + k3;
 }
 
+// One cell of the plane above the threshold (MODE 1; same layout as fdas_candidate in include/fdas.h)
+struct Candidate {
+    long long col;
+    int row;
+    float power;
+};
+
 struct KernelParams {
     const float2 *spectrum;   // N complex64
-    float *plane;             // K x ncols
+    float *plane;             // K x ncols (MODE 1: null; cells are addressed relative to it, never stored)
+    Candidate *cands;         // MODE 1: candidate list, `capacity` entries
+    unsigned long long *count; // MODE 1: number of cells found (may exceed capacity)
+    long long capacity;
+    float threshold;          // MODE 1: keep cells with P > threshold
     const float4 *hperm;      // [npairs][PTS/2][T] float4 = 2 complex H values (z <= 0 rows)
     const float2 *wtab;       // exp(-2 pi i j / L), j < L   (seglen 8192: L = 4096 here)
     const float2 *wtab2;      // seglen 8192 only: exp(-2 pi i j / 8192), j < 8192
@@ -295,6 +306,43 @@ __device__ __forceinline__ void st_stream2_if(float *p, float a, float b, unsign
                  ::"l"(p), "f"(a), "f"(b), "r"(pred) : "memory");
 }
 
+// Plane sink.  MODE 0 (fdas_execute): streaming store of the cell.  MODE 1 (fdas_execute_threshold,
+// PAPER.md:73 "comparing the resulting Fourier power to a pre-calculated threshold", :331): the plane
+// never reaches memory; a cell above the threshold is appended to the candidate list (rare path:
+// its row / column are recovered from the address the store would have used).
+__device__ __noinline__ void push_candidate(const KernelParams &prm, const float *p, float v)
+{
+    const long long idx = p - prm.plane;
+    const long long row = idx / prm.ncols;
+    const unsigned long long slot = atomicAdd(prm.count, 1ull);
+    if (slot < (unsigned long long)prm.capacity) {
+        Candidate c;
+        c.col = idx - row * prm.ncols;
+        c.row = (int)row;
+        c.power = v;
+        prm.cands[slot] = c;
+    }
+}
+template <int MODE>
+__device__ __forceinline__ void emit_if(const KernelParams &prm, float *p, float v, unsigned pred)
+{
+    if constexpr (MODE == 0) {
+        st_stream_if(p, v, pred);
+    } else {
+        if (pred && v > prm.threshold) push_candidate(prm, p, v);
+    }
+}
+template <int MODE>
+__device__ __forceinline__ void emit2_if(const KernelParams &prm, float *p, float a, float b, unsigned pred)
+{
+    if constexpr (MODE == 0) {
+        st_stream2_if(p, a, b, pred);
+    } else {
+        if (pred && a > prm.threshold) push_candidate(prm, p, a);
+        if (pred && b > prm.threshold) push_candidate(prm, p + 1, b);
+    }
+}
+
 // ---- split-phase CTA barrier on shared memory (mbarrier): arrive now, wait later
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
@@ -321,7 +369,7 @@ struct Pending {
     bool on;
 };
 
-template <int L>
+template <int L, int MODE = 0>
 __device__ __forceinline__ void flush_edges(const KernelParams &prm, const ThreadMap<L> &tm, const float4 *edges,
                                             Pending<L> &pd)
 {
@@ -341,15 +389,17 @@ __device__ __forceinline__ void flush_edges(const KernelParams &prm, const Threa
     const int n = n1 * G::Q + 32 * tm.warp + 31;
     const long long col = pd.col0 + n;
     const int row = lo ? pd.pair : prm.ntemplates - 1 - pd.pair;
-    st_stream2_if(prm.plane + (size_t)row * prm.ncols + 2 * col, pw, ph,
-                  n >= prm.overlap && n < prm.overlap + prm.useful && col < prm.nbins);
+    // MODE 1: the z = 0 slot's q row is its p row again -- report it once
+    const bool dup = MODE != 0 && !lo && row == pd.pair;
+    emit2_if<MODE>(prm, prm.plane + (size_t)row * prm.ncols + 2 * col, pw, ph,
+                   n >= prm.overlap && n < prm.overlap + prm.useful && col < prm.nbins && !dup);
     pd.on = false;
 }
 
 // Persistent fused kernel.  Work = nseg * npairs (segment, template-slot) units, split into
 // gridDim.x equal contiguous ranges (segment-major), so each CTA redoes at most one extra
 // forward FFT at a range boundary and every CTA gets the same number of inverse FFT pairs.
-template <int L, bool INTERBIN, int MINB>
+template <int L, bool INTERBIN, int MINB, int MODE = 0>
 __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const KernelParams prm)
 {
     using G = Geo<L>;
@@ -407,7 +457,7 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
         if (!have_q3) {
             // first unit of a segment for this CTA: the pipeline is drained; forward transform
             __syncthreads();                                  // nobody reads E1 / E2 / edges any more
-            if (INTERBIN && pend.on) flush_edges<L>(prm, tm, edges, pend);
+            if (INTERBIN && pend.on) flush_edges<L, MODE>(prm, tm, edges, pend);
             fwd_f1<L>(prm.spectrum, prm.nbins, seg * prm.useful - prm.overlap, prm.wtab, tm, e1base);
             __syncthreads();
             fwd_f2<L>(prm.wtab, tm, e1base, e2.re);
@@ -432,7 +482,7 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
         }
         mbar_wait(&mbar[par], (c >> 1) & 1);                  // all of E1[par] is written
 
-        if (INTERBIN && pend.on) flush_edges<L>(prm, tm, edges, pend);   // every warp is past Q1(c-1)
+        if (INTERBIN && pend.on) flush_edges<L, MODE>(prm, tm, edges, pend);   // every warp is past Q1(c-1)
 
         const int row_p = pair;                         // z <= 0
         const int row_q = prm.ntemplates - 1 - pair;    // z >= 0 (same row for the z = 0 slot)
@@ -446,15 +496,16 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
                 if (col0 + n1 * G::Q + tid >= prm.nbins) vm &= ~(1u << n1);
         }
         // The z = 0 slot has row_q == row_p and q == p bit for bit (H_0 is real), so its second
-        // store rewrites the same value: no special case.
+        // store rewrites the same value: no special case (MODE 1 reports the cell once: vq = 0).
+        const unsigned qon = (MODE != 0 && row_q == row_p) ? 0u : ~0u;
         if constexpr (!INTERBIN) {
             float *bp = prm.plane + (size_t)row_p * prm.ncols + (col0 + tid);
             float *bq = prm.plane + (size_t)row_q * prm.ncols + (col0 + tid);
 #pragma unroll
             for (int n1 = 0; n1 < 16; ++n1) {
                 const float2 pw = power2(y[n1]);
-                st_stream_if(bp + n1 * G::Q, pw.x, vm & (1u << n1));
-                st_stream_if(bq + n1 * G::Q, pw.y, vm & (1u << n1));
+                emit_if<MODE>(prm, bp + n1 * G::Q, pw.x, vm & (1u << n1));
+                emit_if<MODE>(prm, bq + n1 * G::Q, pw.y, vm & qon & (1u << n1));
             }
         } else {
             // lanes 0 and 31 post their y to the mailbox; lane 31's cells (power and half-bin) are
@@ -477,8 +528,8 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
                                                   __shfl_down_sync(0xffffffffu, y[n1].im.y, 1)));
                 const float2 pw = power2(y[n1]);
                 const float2 ph = mul2(power2(d), bc2(IB));
-                st_stream2_if(bp + 2 * n1 * G::Q, pw.x, ph.x, vm & (1u << n1));
-                st_stream2_if(bq + 2 * n1 * G::Q, pw.y, ph.y, vm & (1u << n1));
+                emit2_if<MODE>(prm, bp + 2 * n1 * G::Q, pw.x, ph.x, vm & (1u << n1));
+                emit2_if<MODE>(prm, bq + 2 * n1 * G::Q, pw.y, ph.y, vm & qon & (1u << n1));
             }
             pend.col0 = col0;
             pend.pair = pair;
@@ -493,7 +544,7 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
     }
     if (INTERBIN && pend.on) {
         __syncthreads();
-        flush_edges<L>(prm, tm, edges, pend);
+        flush_edges<L, MODE>(prm, tm, edges, pend);
     }
 }
 

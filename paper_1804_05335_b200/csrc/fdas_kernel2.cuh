@@ -190,7 +190,7 @@ __device__ __forceinline__ void inv_q3_q2(const float2 (&xh)[Geo<L>::PTS], const
     q3_tail_q2<L>(a, tw, tm, out);
 }
 
-template <int L, bool INTERBIN, int MINB>
+template <int L, bool INTERBIN, int MINB, int MODE = 0>
 __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const KernelParams prm)
 {
     using G = Geo<L>;
@@ -252,7 +252,7 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
         inv_q3_q2<L>(xh, h4, tw, tm, o);
         fetch_h();
         if (u >= 2) mbar_wait(&empty[u & 1], ((u >> 1) - 1) & 1);   // every warp has consumed unit u-2
-        if (INTERBIN && pend[u & 1].on) flush_edges<L>(prm, tm, edges, pend[u & 1]);
+        if (INTERBIN && pend[u & 1].on) flush_edges<L, MODE>(prm, tm, edges, pend[u & 1]);
         const XBuf e1 = e1buf(u);
 #pragma unroll
         for (int n2 = 0; n2 < 16; ++n2) e1.put(tm.e1_q2 + n2 * G::R3, o[n2]);
@@ -266,6 +266,7 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
         const int row_p = qpair;                        // z <= 0
         const int row_q = prm.ntemplates - 1 - qpair;   // z >= 0 (same row for the z = 0 slot)
         const long long col0 = seg * prm.useful - prm.overlap;  // column of local index 0
+        const unsigned qon = (MODE != 0 && row_q == row_p) ? 0u : ~0u;   // MODE 1: z = 0 cell reported once
         cpk y[16];
 #pragma unroll
         for (int k1 = 0; k1 < 16; ++k1) y[k1] = e1.get(k1 * G::S1 + tid);
@@ -284,8 +285,8 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
 #pragma unroll
             for (int n1 = 0; n1 < 16; ++n1) {
                 const float2 pw = power2(y[n1]);
-                st_stream_if(bp + n1 * G::Q, pw.x, vm & (1u << n1));
-                st_stream_if(bq + n1 * G::Q, pw.y, vm & (1u << n1));
+                emit_if<MODE>(prm, bp + n1 * G::Q, pw.x, vm & (1u << n1));
+                emit_if<MODE>(prm, bq + n1 * G::Q, pw.y, vm & qon & (1u << n1));
             }
         } else {
             const int par = q & 1;
@@ -308,8 +309,8 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
                                                   __shfl_down_sync(0xffffffffu, y[n1].im.y, 1)));
                 const float2 pw = power2(y[n1]);
                 const float2 ph = mul2(power2(d), bc2(IB));
-                st_stream2_if(bp + 2 * n1 * G::Q, pw.x, ph.x, vm & (1u << n1));
-                st_stream2_if(bq + 2 * n1 * G::Q, pw.y, ph.y, vm & (1u << n1));
+                emit2_if<MODE>(prm, bp + 2 * n1 * G::Q, pw.x, ph.x, vm & (1u << n1));
+                emit2_if<MODE>(prm, bq + 2 * n1 * G::Q, pw.y, ph.y, vm & qon & (1u << n1));
             }
             pend[par].col0 = col0;
             pend[par].pair = qpair;
@@ -326,8 +327,8 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
         if (first) {
             __syncthreads();                                   // every earlier unit is consumed
             if (INTERBIN) {
-                if (pend[0].on) flush_edges<L>(prm, tm, edges, pend[0]);
-                if (pend[1].on) flush_edges<L>(prm, tm, edges, pend[1]);
+                if (pend[0].on) flush_edges<L, MODE>(prm, tm, edges, pend[0]);
+                if (pend[1].on) flush_edges<L, MODE>(prm, tm, edges, pend[1]);
             }
             float2 *scr = e1base + 2 * G::E1_ELEMS;            // second buffer: F2 -> F3 scratch
             fwd_f1<L>(prm.spectrum, prm.nbins, seg * prm.useful - prm.overlap, prm.wtab, tm, e1base);
@@ -348,8 +349,8 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
     }
     if (INTERBIN) {
         __syncthreads();
-        if (pend[0].on) flush_edges<L>(prm, tm, edges, pend[0]);
-        if (pend[1].on) flush_edges<L>(prm, tm, edges, pend[1]);
+        if (pend[0].on) flush_edges<L, MODE>(prm, tm, edges, pend[0]);
+        if (pend[1].on) flush_edges<L, MODE>(prm, tm, edges, pend[1]);
     }
 }
 

@@ -77,7 +77,7 @@ __device__ __forceinline__ void inv_q3_8k(const float2 *xs_lo, const float2 *xs_
     }
 }
 
-template <int MINB>
+template <int MINB, int MODE = 0>
 __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelParams prm)
 {
     using G = Geo<4096>;
@@ -212,11 +212,12 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
         }
         float *bp = prm.plane + (size_t)row_p * prm.ncols + (col0 + 2 * tid + par);
         float *bq = prm.plane + (size_t)row_q * prm.ncols + (col0 + 2 * tid + par);
+        const unsigned qon = (MODE != 0 && row_q == row_p) ? 0u : ~0u;   // MODE 1: z = 0 cell reported once
 #pragma unroll
         for (int n1 = 0; n1 < 16; ++n1) {
             const float2 pw = power2(y[n1]);
-            st_stream_if(bp + 2 * n1 * G::Q, pw.x, vm & (1u << n1));
-            st_stream_if(bq + 2 * n1 * G::Q, pw.y, vm & (1u << n1));
+            emit_if<MODE>(prm, bp + 2 * n1 * G::Q, pw.x, vm & (1u << n1));
+            emit_if<MODE>(prm, bq + 2 * n1 * G::Q, pw.y, vm & qon & (1u << n1));
         }
         __syncwarp();
         if (par == 1 && ++pair == prm.npairs) {

@@ -18,7 +18,8 @@ STATUS_NAMES = {0: "FDAS_OK", 1: "FDAS_ERR_INVALID_ARG", 2: "FDAS_ERR_UNSUPPORTE
                 4: "FDAS_ERR_ALIGNMENT", 5: "FDAS_ERR_CUDA", 6: "FDAS_ERR_NOMEM"}
 
 # every symbol include/fdas.h declares
-EXPORTS = ["fdas_plan_create", "fdas_make_templates", "fdas_execute", "fdas_execute_host", "fdas_destroy",
+EXPORTS = ["fdas_plan_create", "fdas_make_templates", "fdas_execute", "fdas_execute_host", "fdas_execute_threshold",
+           "fdas_destroy",
            "fdas_plan_info", "fdas_get_taps", "fdas_get_template_spectrum", "fdas_measure_fp32_peak", "fdas_probe_pipes",
            "fdas_launch_count", "fdas_status_string", "fdas_last_error"]
 
@@ -54,6 +55,7 @@ def _load() -> ctypes.CDLL:
     lib.fdas_make_templates.argtypes = [vp, vp]
     lib.fdas_execute.argtypes = [vp, vp, vp, vp]
     lib.fdas_execute_host.argtypes = [vp, vp, vp, vp]
+    lib.fdas_execute_threshold.argtypes = [vp, vp, vp, ctypes.c_float, vp, i64, vp]
     lib.fdas_destroy.argtypes = [vp]
     lib.fdas_plan_info.argtypes = [vp, ctypes.POINTER(FdasInfo)]
     lib.fdas_get_taps.argtypes = [vp, i32, vp, ctypes.POINTER(i32)]
@@ -123,6 +125,13 @@ def fdas_execute_host(plan: int, stream, h_spectrum, h_fdot_plane) -> None:
            "fdas_execute_host", plan)
 
 
+def fdas_execute_threshold(plan: int, stream, d_spectrum, threshold: float, d_cands, capacity: int, d_count) -> None:
+    """d_cands: device buffer of `capacity` 16-byte fdas_candidate records {int64 col, int32 row, float power};
+    d_count: device uint64 (zeroed by the call)."""
+    _check(lib.fdas_execute_threshold(plan, _stream(stream), _ptr(d_spectrum), float(threshold), _ptr(d_cands),
+                                      int(capacity), _ptr(d_count)), "fdas_execute_threshold", plan)
+
+
 def fdas_destroy(plan: int) -> None:
     _check(lib.fdas_destroy(plan), "fdas_destroy")
 
@@ -172,6 +181,10 @@ def fdas_launch_count() -> int:
     return int(lib.fdas_launch_count())
 
 
+# numpy view of a candidate buffer copied to the host (marshalling only)
+CANDIDATE_DTYPE = [("col", "<i8"), ("row", "<i4"), ("power", "<f4")]
+
+
 # ---- small convenience wrapper (still marshalling only) --------------------------------------
 class Plan:
     """RAII wrapper: Plan(nbins, zmax, dz, seglen, interbin).make_templates().execute(stream, spec, plane)."""
@@ -186,6 +199,9 @@ class Plan:
 
     def execute(self, stream, d_spectrum, d_plane):
         fdas_execute(self.handle, stream, d_spectrum, d_plane)
+
+    def execute_threshold(self, stream, d_spectrum, threshold, d_cands, capacity, d_count):
+        fdas_execute_threshold(self.handle, stream, d_spectrum, threshold, d_cands, capacity, d_count)
 
     def execute_host(self, stream, h_spectrum, h_plane):
         fdas_execute_host(self.handle, stream, h_spectrum, h_plane)

@@ -354,6 +354,32 @@ def main():
     e2e_value = world * args.e2e_steps * w["cells"] / (e2e_ms * 1e-3)
     checksum = float(h_out[K // 2, : min(1024, ncols)].sum())
 
+    # ---- threshold-search mode: the same fused kernel with a candidate
+    # sink instead of the plane store; reported beside the headline, never instead of it
+    thr_val, thr_cap = 16.0, 1 << 20
+    d_cands = torch.empty(thr_cap * 16, dtype=torch.uint8, device=dev)
+    d_count = torch.zeros(1, dtype=torch.int64, device=dev)
+    h_cands = torch.empty(thr_cap * 16, dtype=torch.uint8).pin_memory()
+    h_count = torch.zeros(1, dtype=torch.int64).pin_memory()
+    with torch.cuda.stream(stream):
+        for i in range(3):
+            plan.execute_threshold(stream, d_in[i % nin], thr_val, d_cands, thr_cap, d_count)
+        t0e, t1e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0e.record(stream)
+        for i in range(args.steps):
+            plan.execute_threshold(stream, d_in[i % nin], thr_val, d_cands, thr_cap, d_count)
+        t1e.record(stream)
+    stream.synchronize()
+    thr_ms = dist.max_over_ranks(t0e.elapsed_time(t1e), dev) / args.steps
+    plan.execute_threshold_host(stream, h_in, thr_val, h_cands, thr_cap, h_count)      # warm-up (staging)
+    t0e.record(stream)
+    for i in range(args.e2e_steps):
+        plan.execute_threshold_host(stream, h_in, thr_val, h_cands, thr_cap, h_count)
+    t1e.record(stream)
+    stream.synchronize()
+    thr_e2e_ms = dist.max_over_ranks(t0e.elapsed_time(t1e), dev) / args.e2e_steps
+    thr_found = int(h_count.item())
+
     fp32_probe = fdas.fdas_measure_fp32_peak(stream, 4000) if rank == 0 else None
 
     # ---- same-box comparator: the paper's unfused cuFFT pipeline (harness-side, N = 1 only)
@@ -406,6 +432,14 @@ def main():
             "clocks": clocks,
             "roofline": roof,
         }
+        out["threshold_search"] = {
+            "what": "fdas_execute_threshold: same fused kernel, cells with P > threshold appended to a candidate "
+                    "list instead of the plane store (paper's stated next step, PAPER.md:73, :331)",
+            "threshold": thr_val, "candidates_found": thr_found, "ms_per_step": thr_ms,
+            "value": world * w["cells"] / (thr_ms * 1e-3), "unit": "cells searched/s",
+            "e2e": {"value": world * w["cells"] / (thr_e2e_ms * 1e-3), "unit": "cells searched/s",
+                    "ms_per_step": thr_e2e_ms, "h2d_bytes_per_step": 8 * N,
+                    "d2h_bytes_per_step": 8 + 16 * min(thr_found, thr_cap)}}
         if cufft_ms is not None:
             out["cufft_unfused"] = {"ms_per_step": cufft_ms, "value": w["cells"] / (cufft_ms * 1e-3), "unit": UNIT,
                                     "fused_speedup": cufft_ms / (avg_kernel_s * 1e3),

@@ -137,6 +137,15 @@ typedef struct fdas_candidate {
 fdas_status fdas_execute_threshold(fdas_plan *plan, void *stream, const void *d_spectrum, float threshold,
                                    fdas_candidate *d_cands, int64_t capacity, uint64_t *d_count);
 
+/*
+ * End-to-end threshold search for HOST buffers: copies `h_spectrum` to a plan-owned device buffer,
+ * runs fdas_execute_threshold, copies the count to *h_count, then the first min(*h_count, capacity)
+ * candidates to `h_cands`, and synchronises `stream`.  Staging buffers are allocated on first use
+ * (the candidate buffer grows when `capacity` does) and freed by fdas_destroy.
+ */
+fdas_status fdas_execute_threshold_host(fdas_plan *plan, void *stream, const void *h_spectrum, float threshold,
+                                        fdas_candidate *h_cands, int64_t capacity, uint64_t *h_count);
+
 /* Free the plan and everything it owns.  fdas_destroy(NULL) is a no-op returning FDAS_OK. */
 fdas_status fdas_destroy(fdas_plan *plan);
 

@@ -27,6 +27,9 @@ struct fdas_plan {
     float2 *d_wtab2;     // seglen 8192 only: 8192 entries
     float2 *d_stage_in;  // fdas_execute_host staging (lazy)
     float *d_stage_out;
+    fdas_candidate *d_stage_cands;   // fdas_execute_threshold_host staging (lazy, grows with capacity)
+    int64_t stage_cands_cap;
+    unsigned long long *d_stage_count;
     void (*kernel)(const KernelParams);
     void (*kernel_thr)(const KernelParams);   // MODE 1: threshold search instead of the plane store
     char err[256];
@@ -311,9 +314,53 @@ fdas_status fdas_execute_host(fdas_plan *p, void *stream, const void *h_spectrum
     return FDAS_OK;
 }
 
+fdas_status fdas_execute_threshold_host(fdas_plan *p, void *stream, const void *h_spectrum, float threshold,
+                                        fdas_candidate *h_cands, int64_t capacity, uint64_t *h_count)
+{
+    if (!p || !h_spectrum || !h_count || capacity < 0 || (capacity > 0 && !h_cands)) return FDAS_ERR_INVALID_ARG;
+    if (!p->ready) return FDAS_ERR_NOT_READY;
+    const fdas_info &I = p->info;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!p->d_stage_in && cudaMalloc(&p->d_stage_in, (size_t)I.nbins * sizeof(float2)) != cudaSuccess) {
+        cudaGetLastError();
+        return FDAS_ERR_NOMEM;
+    }
+    if (!p->d_stage_count && cudaMalloc(&p->d_stage_count, sizeof(unsigned long long)) != cudaSuccess) {
+        cudaGetLastError();
+        return FDAS_ERR_NOMEM;
+    }
+    if (capacity > p->stage_cands_cap) {
+        FDAS_CUDA(p, cudaStreamSynchronize(st));
+        cudaFree(p->d_stage_cands);
+        p->d_stage_cands = nullptr;
+        p->stage_cands_cap = 0;
+        if (cudaMalloc(&p->d_stage_cands, (size_t)capacity * sizeof(fdas_candidate)) != cudaSuccess) {
+            cudaGetLastError();
+            return FDAS_ERR_NOMEM;
+        }
+        p->stage_cands_cap = capacity;
+    }
+    FDAS_CUDA(p, cudaMemcpyAsync(p->d_stage_in, h_spectrum, (size_t)I.nbins * sizeof(float2),
+                                 cudaMemcpyHostToDevice, st));
+    fdas_status s = fdas_execute_threshold(p, stream, p->d_stage_in, threshold, p->d_stage_cands, capacity,
+                                           (uint64_t *)p->d_stage_count);
+    if (s != FDAS_OK) return s;
+    FDAS_CUDA(p, cudaMemcpyAsync(h_count, p->d_stage_count, sizeof(uint64_t), cudaMemcpyDeviceToHost, st));
+    FDAS_CUDA(p, cudaStreamSynchronize(st));
+    const uint64_t nvalid = *h_count < (uint64_t)capacity ? *h_count : (uint64_t)capacity;
+    if (nvalid) {
+        FDAS_CUDA(p, cudaMemcpyAsync(h_cands, p->d_stage_cands, (size_t)nvalid * sizeof(fdas_candidate),
+                                     cudaMemcpyDeviceToHost, st));
+        FDAS_CUDA(p, cudaStreamSynchronize(st));
+    }
+    return FDAS_OK;
+}
+
 fdas_status fdas_destroy(fdas_plan *p)
 {
     if (!p) return FDAS_OK;
+    cudaFree(p->d_stage_cands);
+    cudaFree(p->d_stage_count);
     cudaFree(p->d_taps);
     cudaFree(p->d_hperm);
     cudaFree(p->d_wtab);

@@ -343,6 +343,77 @@ __device__ __forceinline__ void emit2_if(const KernelParams &prm, float *p, floa
     }
 }
 
+// Epilogue of one unit: power (a6) and interbin (a7) of this thread's 16 outputs y[n1*Q + tid] of the
+// (p, q) pair, handed to the plane sink (a8).  bp / bq: address of the n1 = 0 cell in rows p / q; the n1
+// step is STRIDE*Q cells (2*Q interbinned).  vm / vmq: valid-output masks of the two rows.
+// MODE 1 first takes the maximum over the unit's cells and leaves unless some cell of the WARP passes the
+// threshold (warp-uniform, so the interbin shuffles of the slow path stay converged): the common case
+// costs no branch per cell.  Masked-out cells take part in the maximum; that can only cost time.
+template <int L, bool INTERBIN, int MODE, int STRIDE>
+__device__ __forceinline__ void emit_cells(const KernelParams &prm, const cpk (&y)[16], float *bp, float *bq,
+                                           unsigned vm, unsigned vmq)
+{
+    constexpr int Q = Geo<L>::Q;
+    constexpr float IB = 0.61685027506808491367715568749226f; // (pi/4)^2, eq. 4 squared
+#pragma unroll
+    for (int n1 = 0; n1 < 16; ++n1) {
+        const float2 pw = power2(y[n1]);
+        if constexpr (!INTERBIN) {
+            emit_if<MODE>(prm, bp + STRIDE * n1 * Q, pw.x, vm & (1u << n1));
+            emit_if<MODE>(prm, bq + STRIDE * n1 * Q, pw.y, vmq & (1u << n1));
+        } else {
+            cpk d;                                   // y[n] - y[n+1], neighbour from lane + 1
+            d.re = sub2(y[n1].re, make_float2(__shfl_down_sync(0xffffffffu, y[n1].re.x, 1),
+                                              __shfl_down_sync(0xffffffffu, y[n1].re.y, 1)));
+            d.im = sub2(y[n1].im, make_float2(__shfl_down_sync(0xffffffffu, y[n1].im.x, 1),
+                                              __shfl_down_sync(0xffffffffu, y[n1].im.y, 1)));
+            const float2 ph = mul2(power2(d), bc2(IB));
+            emit2_if<MODE>(prm, bp + 2 * n1 * Q, pw.x, ph.x, vm & (1u << n1));
+            emit2_if<MODE>(prm, bq + 2 * n1 * Q, pw.y, ph.y, vmq & (1u << n1));
+        }
+    }
+}
+// MODE 1 slow path, out of line (its register needs and calls stay out of the main loop); entered by whole
+// warps only, so the interbin shuffles are converged.
+template <int L, bool INTERBIN, int STRIDE>
+__device__ __noinline__ void emit_cells_rare(const KernelParams &prm, const cpk (&y)[16], float *bp, float *bq,
+                                             unsigned vm, unsigned vmq)
+{
+    emit_cells<L, INTERBIN, 1, STRIDE>(prm, y, bp, bq, vm, vmq);
+}
+
+template <int L, bool INTERBIN, int MODE, int STRIDE>
+__device__ __forceinline__ void emit_unit(const KernelParams &prm, const cpk (&y)[16], float *bp, float *bq,
+                                          unsigned vm, unsigned vmq)
+{
+    if constexpr (MODE == 0) {
+        emit_cells<L, INTERBIN, 0, STRIDE>(prm, y, bp, bq, vm, vmq);
+    } else {
+        constexpr float IB = 0.61685027506808491367715568749226f;
+        float2 mx = power2(y[0]);
+#pragma unroll
+        for (int n1 = 0; n1 < 16; ++n1) {
+            const float2 pw = power2(y[n1]);
+            mx = make_float2(fmaxf(mx.x, pw.x), fmaxf(mx.y, pw.y));
+            if constexpr (INTERBIN) {
+                cpk d;
+                d.re = sub2(y[n1].re, make_float2(__shfl_down_sync(0xffffffffu, y[n1].re.x, 1),
+                                                  __shfl_down_sync(0xffffffffu, y[n1].re.y, 1)));
+                d.im = sub2(y[n1].im, make_float2(__shfl_down_sync(0xffffffffu, y[n1].im.x, 1),
+                                                  __shfl_down_sync(0xffffffffu, y[n1].im.y, 1)));
+                const float2 ph = mul2(power2(d), bc2(IB));
+                mx = make_float2(fmaxf(mx.x, ph.x), fmaxf(mx.y, ph.y));
+            }
+        }
+        if (__any_sync(0xffffffffu, fmaxf(mx.x, mx.y) > prm.threshold)) {
+            cpk ys[16];                              // a copy in local memory: y itself stays in registers
+#pragma unroll
+            for (int n1 = 0; n1 < 16; ++n1) ys[n1] = y[n1];
+            emit_cells_rare<L, INTERBIN, STRIDE>(prm, ys, bp, bq, vm, vmq);
+        }
+    }
+}
+
 // ---- split-phase CTA barrier on shared memory (mbarrier): arrive now, wait later
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
@@ -449,7 +520,6 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
         if (nn >= prm.overlap && nn < prm.overlap + prm.useful) vmask |= 1u << n1;
     }
 
-    constexpr float IB = 0.61685027506808491367715568749226f; // (pi/4)^2, eq. 4 squared
     Pending<L> pend{0, 0, 0, false};
     bool have_q3 = false;
 
@@ -501,12 +571,7 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
         if constexpr (!INTERBIN) {
             float *bp = prm.plane + (size_t)row_p * prm.ncols + (col0 + tid);
             float *bq = prm.plane + (size_t)row_q * prm.ncols + (col0 + tid);
-#pragma unroll
-            for (int n1 = 0; n1 < 16; ++n1) {
-                const float2 pw = power2(y[n1]);
-                emit_if<MODE>(prm, bp + n1 * G::Q, pw.x, vm & (1u << n1));
-                emit_if<MODE>(prm, bq + n1 * G::Q, pw.y, vm & qon & (1u << n1));
-            }
+            emit_unit<L, false, MODE, 1>(prm, y, bp, bq, vm, vm & qon);
         } else {
             // lanes 0 and 31 post their y to the mailbox; lane 31's cells (power and half-bin) are
             // written one unit later by flush_edges, every other lane stores (P[n], P[n+1/2]) now
@@ -519,18 +584,7 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
             float *bp = prm.plane + (size_t)row_p * prm.ncols + 2 * (col0 + tid);
             float *bq = prm.plane + (size_t)row_q * prm.ncols + 2 * (col0 + tid);
             if (tm.lane == 31) vm = 0;
-#pragma unroll
-            for (int n1 = 0; n1 < 16; ++n1) {
-                cpk d;                                   // y[n] - y[n+1], neighbour from lane + 1
-                d.re = sub2(y[n1].re, make_float2(__shfl_down_sync(0xffffffffu, y[n1].re.x, 1),
-                                                  __shfl_down_sync(0xffffffffu, y[n1].re.y, 1)));
-                d.im = sub2(y[n1].im, make_float2(__shfl_down_sync(0xffffffffu, y[n1].im.x, 1),
-                                                  __shfl_down_sync(0xffffffffu, y[n1].im.y, 1)));
-                const float2 pw = power2(y[n1]);
-                const float2 ph = mul2(power2(d), bc2(IB));
-                emit2_if<MODE>(prm, bp + 2 * n1 * G::Q, pw.x, ph.x, vm & (1u << n1));
-                emit2_if<MODE>(prm, bq + 2 * n1 * G::Q, pw.y, ph.y, vm & qon & (1u << n1));
-            }
+            emit_unit<L, true, MODE, 1>(prm, y, bp, bq, vm, vm & qon);
             pend.col0 = col0;
             pend.pair = pair;
             pend.par = par;

@@ -240,7 +240,6 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
         if (nn >= prm.overlap && nn < prm.overlap + prm.useful) vmask |= 1u << n1;
     }
 
-    constexpr float IB = 0.61685027506808491367715568749226f; // (pi/4)^2, eq. 4 squared
     Pending<L> pend[2] = {{0, 0, 0, false}, {0, 0, 1, false}};
     auto e1buf = [&](int u) {
         float2 *b = e1base + (u & 1) * 2 * G::E1_ELEMS;
@@ -282,12 +281,7 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
         if constexpr (!INTERBIN) {
             float *bp = prm.plane + (size_t)row_p * prm.ncols + (col0 + tid);
             float *bq = prm.plane + (size_t)row_q * prm.ncols + (col0 + tid);
-#pragma unroll
-            for (int n1 = 0; n1 < 16; ++n1) {
-                const float2 pw = power2(y[n1]);
-                emit_if<MODE>(prm, bp + n1 * G::Q, pw.x, vm & (1u << n1));
-                emit_if<MODE>(prm, bq + n1 * G::Q, pw.y, vm & qon & (1u << n1));
-            }
+            emit_unit<L, false, MODE, 1>(prm, y, bp, bq, vm, vm & qon);
         } else {
             const int par = q & 1;
             float4 *eb = edges + par * (2 * G::W * 16) + (tm.lane == 0 ? G::W * 16 : 0) + tm.warp * 16;
@@ -300,18 +294,7 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
             float *bp = prm.plane + (size_t)row_p * prm.ncols + 2 * (col0 + tid);
             float *bq = prm.plane + (size_t)row_q * prm.ncols + 2 * (col0 + tid);
             if (tm.lane == 31) vm = 0;
-#pragma unroll
-            for (int n1 = 0; n1 < 16; ++n1) {
-                cpk d;                                   // y[n] - y[n+1], neighbour from lane + 1
-                d.re = sub2(y[n1].re, make_float2(__shfl_down_sync(0xffffffffu, y[n1].re.x, 1),
-                                                  __shfl_down_sync(0xffffffffu, y[n1].re.y, 1)));
-                d.im = sub2(y[n1].im, make_float2(__shfl_down_sync(0xffffffffu, y[n1].im.x, 1),
-                                                  __shfl_down_sync(0xffffffffu, y[n1].im.y, 1)));
-                const float2 pw = power2(y[n1]);
-                const float2 ph = mul2(power2(d), bc2(IB));
-                emit2_if<MODE>(prm, bp + 2 * n1 * G::Q, pw.x, ph.x, vm & (1u << n1));
-                emit2_if<MODE>(prm, bq + 2 * n1 * G::Q, pw.y, ph.y, vm & qon & (1u << n1));
-            }
+            emit_unit<L, true, MODE, 1>(prm, y, bp, bq, vm, vm & qon);
             pend[par].col0 = col0;
             pend[par].pair = qpair;
             pend[par].par = par;

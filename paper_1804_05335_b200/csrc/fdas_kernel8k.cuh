@@ -213,12 +213,7 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
         float *bp = prm.plane + (size_t)row_p * prm.ncols + (col0 + 2 * tid + par);
         float *bq = prm.plane + (size_t)row_q * prm.ncols + (col0 + 2 * tid + par);
         const unsigned qon = (MODE != 0 && row_q == row_p) ? 0u : ~0u;   // MODE 1: z = 0 cell reported once
-#pragma unroll
-        for (int n1 = 0; n1 < 16; ++n1) {
-            const float2 pw = power2(y[n1]);
-            emit_if<MODE>(prm, bp + 2 * n1 * G::Q, pw.x, vm & (1u << n1));
-            emit_if<MODE>(prm, bq + 2 * n1 * G::Q, pw.y, vm & qon & (1u << n1));
-        }
+        emit_unit<4096, false, MODE, 2>(prm, y, bp, bq, vm, vm & qon);
         __syncwarp();
         if (par == 1 && ++pair == prm.npairs) {
             pair = 0;

@@ -19,6 +19,7 @@ STATUS_NAMES = {0: "FDAS_OK", 1: "FDAS_ERR_INVALID_ARG", 2: "FDAS_ERR_UNSUPPORTE
 
 # every symbol include/fdas.h declares
 EXPORTS = ["fdas_plan_create", "fdas_make_templates", "fdas_execute", "fdas_execute_host", "fdas_execute_threshold",
+           "fdas_execute_threshold_host",
            "fdas_destroy",
            "fdas_plan_info", "fdas_get_taps", "fdas_get_template_spectrum", "fdas_measure_fp32_peak", "fdas_probe_pipes",
            "fdas_launch_count", "fdas_status_string", "fdas_last_error"]
@@ -56,6 +57,7 @@ def _load() -> ctypes.CDLL:
     lib.fdas_execute.argtypes = [vp, vp, vp, vp]
     lib.fdas_execute_host.argtypes = [vp, vp, vp, vp]
     lib.fdas_execute_threshold.argtypes = [vp, vp, vp, ctypes.c_float, vp, i64, vp]
+    lib.fdas_execute_threshold_host.argtypes = [vp, vp, vp, ctypes.c_float, vp, i64, vp]
     lib.fdas_destroy.argtypes = [vp]
     lib.fdas_plan_info.argtypes = [vp, ctypes.POINTER(FdasInfo)]
     lib.fdas_get_taps.argtypes = [vp, i32, vp, ctypes.POINTER(i32)]
@@ -132,6 +134,11 @@ def fdas_execute_threshold(plan: int, stream, d_spectrum, threshold: float, d_ca
                                       int(capacity), _ptr(d_count)), "fdas_execute_threshold", plan)
 
 
+def fdas_execute_threshold_host(plan: int, stream, h_spectrum, threshold: float, h_cands, capacity: int, h_count) -> None:
+    _check(lib.fdas_execute_threshold_host(plan, _stream(stream), _ptr(h_spectrum), float(threshold), _ptr(h_cands),
+                                           int(capacity), _ptr(h_count)), "fdas_execute_threshold_host", plan)
+
+
 def fdas_destroy(plan: int) -> None:
     _check(lib.fdas_destroy(plan), "fdas_destroy")
 
@@ -202,6 +209,9 @@ class Plan:
 
     def execute_threshold(self, stream, d_spectrum, threshold, d_cands, capacity, d_count):
         fdas_execute_threshold(self.handle, stream, d_spectrum, threshold, d_cands, capacity, d_count)
+
+    def execute_threshold_host(self, stream, h_spectrum, threshold, h_cands, capacity, h_count):
+        fdas_execute_threshold_host(self.handle, stream, h_spectrum, threshold, h_cands, capacity, h_count)
 
     def execute_host(self, stream, h_spectrum, h_plane):
         fdas_execute_host(self.handle, stream, h_spectrum, h_plane)

@@ -142,3 +142,23 @@ def test_threshold_full_size_equals_thresholded_plane(cfg):
     for i in rng.choice(count, size=min(count, 40), replace=False):
         ref = orc.plane_cells(spec, zs[rec["row"][i]], [rec["col"][i]], bool(c["interbin"]))[0]
         assert abs(rec["power"][i] - ref) <= 1e-4 * ref and ref > thr - 1e-2
+
+
+def test_threshold_host_end_to_end():
+    """fdas_execute_threshold_host (host buffers in, host candidates out) equals the device entry point."""
+    import torch
+    from paper_1804_05335_b200 import fdas as fd, synthetic as syn
+    n, thr, cap = 1 << 17, 10.0, 1 << 16
+    spec = syn.make_spectrum(n, 4321, [(0.4 * n, 30.0, 15.0)])
+    count_d, rec_d, info = run_threshold(torch, fd, spec, 84.0, 2.0, 2048, 0, thr, cap)
+    with fd.Plan(n, 84.0, 2.0, 2048, 0) as plan:
+        plan.make_templates()
+        h_spec = torch.from_numpy(spec.view(np.float32).reshape(n, 2)).pin_memory()
+        h_cands = torch.zeros(cap * 16, dtype=torch.uint8).pin_memory()
+        h_count = torch.zeros(1, dtype=torch.int64).pin_memory()
+        for capacity in (16, cap):                       # growing capacity re-allocates the staging list
+            plan.execute_threshold_host(torch.cuda.current_stream(), h_spec, thr, h_cands, capacity, h_count)
+            assert int(h_count.item()) == count_d
+        rec = h_cands.numpy().view(fd.CANDIDATE_DTYPE)[:count_d]
+        rec = rec[np.lexsort((rec["col"], rec["row"]))]
+        assert np.array_equal(rec, rec_d)

@@ -73,8 +73,9 @@ kernel_fn select_kernel(int L, bool ib, int mode = 0)
     case 1024: return pick_kernel<1024, 4>(ib, mode);
     case 2048: return pick_kernel<2048, 2>(ib, mode);
     case 4096: return pick_kernel2<4096, 1>(ib, mode);
-    case 8192:                                                            // 2 x 4096, no interbin
-        return ib ? nullptr : mode ? (kernel_fn)fdas_fused_kernel_8k<1, 1> : (kernel_fn)fdas_fused_kernel_8k<1>;
+    case 8192:                                                            // 2 x 4096 (fdas_kernel8k.cuh)
+        if (ib) return mode ? (kernel_fn)fdas_fused_kernel_8k<1, 1, true> : (kernel_fn)fdas_fused_kernel_8k<1, 0, true>;
+        return mode ? (kernel_fn)fdas_fused_kernel_8k<1, 1> : (kernel_fn)fdas_fused_kernel_8k<1>;
     default: return nullptr;
     }
 }

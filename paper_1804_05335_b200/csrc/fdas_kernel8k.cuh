@@ -16,6 +16,15 @@
 //   store: column 2n'+pi of rows -|z| and +|z| (stride-2 streaming stores; the two parities of
 //     a slot follow each other in the same CTA, so L2 merges the sectors).
 //
+// Interbinning (eq. 4) at this segment length: y[n] and y[n+1] belong to different parity
+// sub-units, and neither 64 more registers nor 64 KB more shared memory are there to keep one of them.
+// The difference is taken in the FREQUENCY domain instead (shift theorem):
+//       (pi/4) (y[n] - y[n+1]) = IDFT_8192( X^H[k] * (pi/4)(1 - exp(+2 pi i k / 8192)) )[n]
+// so a slot runs two more sub-units ("half" = 1) whose Q3 input stage scales X^ by that factor (the same
+// for H and conj H) and whose powers are the half-bin cells P[r+1/2] = (pi/4)^2 |y[r] - y[r+1]|^2.  An
+// interbinned 8192 slot therefore costs two plain ones (the paper's own interbinning cost was x1.1-1.6
+// on top of the transform; the shuffle epilogue of the smaller segment lengths is x1.4).
+//
 // With X^ in shared memory only ONE E1 buffer fits: the split-phase `full` barrier is paired
 // with an `empty` barrier (arrive after Q1's loads, wait before Q2's stores).
 #pragma once
@@ -37,16 +46,25 @@ __device__ __forceinline__ constexpr float c32re(int i) { return cosw(i); }
 __device__ __forceinline__ constexpr float c32im(int i) { return sinw(i); }
 
 // Q3 of one parity: products, sum / twiddled difference, inverse DFT16 over k3, twiddle, store E2.
-template <int PARITY>
+template <int PARITY, int HALF = 0>
 __device__ __forceinline__ void inv_q3_8k(const float2 *xs_lo, const float2 *xs_hi, const float4 (&hlo)[8],
                                           const float4 (&hhi)[8], float2 wb, const InvTwiddles<4096> &tw,
-                                          const ThreadMap<4096> &tm, const XBuf &e2)
+                                          const ThreadMap<4096> &tm, const XBuf &e2,
+                                          const float2 *__restrict__ wtab2 = nullptr)
 {
     using G = Geo<4096>;
     cpk a[16];
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
-        const float2 xl = xs_lo[i * G::T + tm.tid], xh = xs_hi[i * G::T + tm.tid];
+        float2 xl = xs_lo[i * G::T + tm.tid], xh = xs_hi[i * G::T + tm.tid];
+        if constexpr (HALF) {
+            // (pi/4)(1 -+ e) with e = exp(+2 pi i k / 8192), k = k1 + 16 k2 + 256 i (the slot of xl; xh is k + 4096)
+            constexpr float S = 0.78539816339744830961566084581988f;
+            const float2 w = wtab2[tm.k1 + 16 * tm.k2m + 256 * i];          // exp(-2 pi i k / 8192)
+            const float2 fl = make_float2(S - S * w.x, S * w.y), fh = make_float2(S + S * w.x, -S * w.y);
+            xl = cmul(xl, fl);
+            xh = cmul(xh, fh);
+        }
         const float4 l4 = hlo[i >> 1], h4 = hhi[i >> 1];
         const float2 hl = (i & 1) ? make_float2(l4.z, l4.w) : make_float2(l4.x, l4.y);
         const float2 hh = (i & 1) ? make_float2(h4.z, h4.w) : make_float2(h4.x, h4.y);
@@ -77,7 +95,7 @@ __device__ __forceinline__ void inv_q3_8k(const float2 *xs_lo, const float2 *xs_
     }
 }
 
-template <int MINB, int MODE = 0>
+template <int MINB, int MODE = 0, bool INTERBIN = false>
 __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelParams prm)
 {
     using G = Geo<4096>;
@@ -139,10 +157,15 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
         if (nn >= ov2 && nn < ov2 + us2) vmask |= 1u << n1;
     }
 
+    // sub-units of a slot: s = par + 2 half (half = 1: the interbin difference transform)
+    constexpr int SUBS = INTERBIN ? 4 : 2;
+    constexpr int CS = INTERBIN ? 2 : 1;              // plane columns per bin
+#define FDAS_Q3_SUB(PAR, HALF) inv_q3_8k<PAR, HALF>(xs_lo, xs_hi, hlo, hhi, wb, tw, tm, e2, prm.wtab2)
     bool have_q3 = false;
-    const int nsub = 2 * n;
+    const int nsub = SUBS * n;
     for (int c = 0; c < nsub; ++c) {
-        const int par = c & 1;
+        const int sub = c % SUBS;
+        const int par = sub & 1, half = sub >> 1;
         if (!have_q3) {
             // first sub-unit of a segment for this CTA (always parity 0): forward transform
             __syncthreads();
@@ -185,14 +208,18 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
         __syncwarp();
 
         // Q3 of the next sub-unit of the same segment
-        have_q3 = (c + 1 < nsub) && (par == 0 || pair + 1 < prm.npairs);
+        have_q3 = (c + 1 < nsub) && (sub + 1 < SUBS || pair + 1 < prm.npairs);
         if (have_q3) {
-            if (par == 0) {
-                inv_q3_8k<1>(xs_lo, xs_hi, hlo, hhi, wb, tw, tm, e2);
-                fetch_h();                                     // next slot's H, one sub-unit ahead
+            if (sub == 0) {
+                FDAS_Q3_SUB(1, 0);
+            } else if (INTERBIN && sub == 1) {
+                FDAS_Q3_SUB(0, 1);
+            } else if (INTERBIN && sub == 2) {
+                FDAS_Q3_SUB(1, 1);
             } else {
-                inv_q3_8k<0>(xs_lo, xs_hi, hlo, hhi, wb, tw, tm, e2);
+                FDAS_Q3_SUB(0, 0);                             // first sub-unit of the next slot
             }
+            if (sub + 2 == SUBS) fetch_h();                    // next slot's H, one sub-unit ahead
         }
         mbar_wait(&mbar[0], c & 1);
 
@@ -210,17 +237,20 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
             for (int n1 = 0; n1 < 16; ++n1)
                 if (col0 + 2 * (n1 * G::Q + tid) + par >= prm.nbins) vm &= ~(1u << n1);
         }
-        float *bp = prm.plane + (size_t)row_p * prm.ncols + (col0 + 2 * tid + par);
-        float *bq = prm.plane + (size_t)row_q * prm.ncols + (col0 + 2 * tid + par);
+        // bin n = 2n' + par -> plane column CS * (col0 + n) + half
+        float *bp = prm.plane + (size_t)row_p * prm.ncols + (CS * (col0 + 2 * tid + par) + half);
+        float *bq = prm.plane + (size_t)row_q * prm.ncols + (CS * (col0 + 2 * tid + par) + half);
         const unsigned qon = (MODE != 0 && row_q == row_p) ? 0u : ~0u;   // MODE 1: z = 0 cell reported once
-        emit_unit<4096, false, MODE, 2>(prm, y, bp, bq, vm, vm & qon);
+        emit_unit<4096, false, MODE, 2 * CS>(prm, y, bp, bq, vm, vm & qon);
         __syncwarp();
-        if (par == 1 && ++pair == prm.npairs) {
+        if (sub == SUBS - 1 && ++pair == prm.npairs) {
             pair = 0;
             ++seg;
         }
     }
 }
+
+#undef FDAS_Q3_SUB
 
 #endif // __CUDACC__
 

@@ -51,7 +51,7 @@ def test_argument_errors_without_device(fd):
     assert lib.fdas_plan_create(ctypes.byref(h), 1024, 20.0, 2.0, 1024, 2) == 1
     assert lib.fdas_plan_create(ctypes.byref(h), 1024, 20.0, 2.0, 1000, 0) == 2      # seglen
     assert lib.fdas_plan_create(ctypes.byref(h), 1024, 2000.0, 2.0, 1024, 0) == 2    # overlap >= seglen/2
-    assert lib.fdas_plan_create(ctypes.byref(h), 1 << 20, 200.0, 2.0, 8192, 1) == 2   # 8192 + interbin
+    assert lib.fdas_plan_create(ctypes.byref(h), 1 << 20, 8100.0, 2.0, 8192, 1) == 2  # overlap >= seglen/2
     assert h.value is None
     assert lib.fdas_destroy(None) == 0
     assert lib.fdas_execute(None, None, None, None) == 1

@@ -187,6 +187,17 @@ def test_seglen_8192_tiny_and_ragged(torch, fd, orc, syn, nbins):
     check_rows(orc, spec, plane, 40.0, 4.0, 0)
 
 
+@pytest.mark.parametrize("nbins,zmax", [(1 << 17, 200.0), (30011, 40.0), (5, 40.0)])
+def test_seglen_8192_interbin(torch, fd, orc, syn, nbins, zmax):
+    """Interbinning at seglen 8192: the half-bin cells come from two more sub-units per slot whose input is
+    scaled by (pi/4)(1 - exp(2 pi i k / L)) (fdas_kernel8k.cuh) -- same eq. 4, checked against the oracle."""
+    chirps = [(0.37 * nbins + 0.5, 0.4 * zmax, 25.0), (nbins - 2.5, -0.8 * zmax, 18.0)] if nbins > 100 else []
+    spec = syn.make_spectrum(nbins, 8192 + nbins, chirps)
+    plane, info = run_gpu(torch, fd, spec, zmax, 4.0, 8192, 1)
+    assert plane.shape == (info["ntemplates"], 2 * nbins) and info["overlap"] >= info["halfwidth"] + 1
+    check_rows(orc, spec, plane, zmax, 4.0, 1)
+
+
 def test_config5_batch_on_one_stream(torch, fd, orc, syn):
     c = syn.CONFIGS[4]
     nb = 3
@@ -241,7 +252,7 @@ def test_deterministic_and_linear(torch, fd, syn):
     assert np.array_equal(p4, 4.0 * p1)                  # power-of-two scaling is exact in fp32
 
 
-@pytest.mark.parametrize("seglen,interbin", [(2048, 0), (2048, 1), (4096, 1), (8192, 0)])
+@pytest.mark.parametrize("seglen,interbin", [(2048, 0), (2048, 1), (4096, 1), (8192, 0), (8192, 1)])
 def test_bitwise_repeatable_all_kernels(torch, fd, syn, seglen, interbin):
     # compute-sanitizer is closed on this pool; a race in the shared-memory exchange pipeline
     # (split-phase mbarriers, per-warp regions, mailbox) would show up as run-to-run differences

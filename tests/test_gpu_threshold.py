@@ -56,6 +56,7 @@ def check_against_oracle(orc, spec, zmax, dz, interbin, thr, rec):
     (1 << 17, 84.0, 4096, 0, 10.0),
     (1 << 17, 84.0, 4096, 1, 10.0),
     (1 << 17, 200.0, 8192, 0, 11.0),
+    (1 << 16, 84.0, 8192, 1, 10.0),
 ])
 def test_threshold_candidates_match_oracle(nbins, zmax, seglen, interbin, thr):
     import torch

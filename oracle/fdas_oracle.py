@@ -22,7 +22,9 @@ sinc/delta special case, brute-force time-domain chirp + DFT, injected-chirp pea
 reversal / shift / linearity invariants, noise statistics, the paper's printed
 interbinning losses, fp64 FFT overlap-save at two segment lengths,
 and a pure-Python triple loop on tiny inputs; the threshold search (`candidates`) by the
-exponential tail law of noise powers, the 0 / +inf thresholds and an injected chirp's cell.
+exponential tail law of noise powers, the 0 / +inf thresholds and an injected chirp's cell; the
+2-bin Fourier interpolation (`interbin = 2`) by a brute-force DFT of a time series zero-padded to
+twice its length, a half-bin tone's full recovery and the time-domain chirp at a half-integer centre.
 No function here is "parity unpinned".
 """
 from __future__ import annotations
@@ -197,29 +199,58 @@ def interbin_from_amplitudes(y_ext: np.ndarray) -> np.ndarray:
     return out
 
 
-def plane_row(spectrum, z: float, interbin: bool = False, m: int | None = None) -> np.ndarray:
-    """One row of the f-fdot plane (float64): N columns, or 2N interbinned."""
+@functools.lru_cache(maxsize=None)
+def _taps2_cached(z: float, m: int) -> np.ndarray:
+    t = response(z, 0.5 * np.arange(-2 * m, 2 * m + 1, dtype=np.float64))
+    t.setflags(write=False)
+    return t
+
+
+def taps2(z: float, m: int | None = None) -> np.ndarray:
+    """Double-resolution template h_z[j/2], j = -2m..+2m (index j + 2m): the template of the 2-bin
+    Fourier interpolation, PAPER.md:89 ("doubling the template and signal resolution")."""
+    if m is None:
+        m = halfwidth(z)
+    return _taps2_cached(float(z), int(m))
+
+
+def interleave_zeros(spectrum) -> np.ndarray:
+    """A2[2k] = A[k], A2[2k+1] = 0: "interleaving zeros prior to the correlations" (PAPER.md:89)."""
     a = _as_c64(spectrum)
+    a2 = np.zeros(2 * a.size, dtype=np.complex64)
+    a2[0::2] = a
+    return a2
+
+
+def plane_row(spectrum, z: float, interbin=False, m: int | None = None) -> np.ndarray:
+    """One row of the f-fdot plane (float64): N columns; 2N interbinned (interbin = 1/True, eq. 4) or
+    with 2-bin Fourier interpolation (interbin = 2, reading R16: the zero-interleaved spectrum
+    correlated with the double-resolution template, column c <-> frequency c/2 bins)."""
+    a = _as_c64(spectrum)
+    if int(interbin) == 2:
+        return power_from_amplitudes(correlate(interleave_zeros(a), taps2(z, m), 0, 2 * a.size))
     h = taps(z, m)
     if interbin:
         return interbin_from_amplitudes(correlate(a, h, 0, a.size + 1))
     return power_from_amplitudes(correlate(a, h, 0, a.size))
 
 
-def plane(spectrum, zmax: float, dz: float, interbin: bool = False) -> np.ndarray:
+def plane(spectrum, zmax: float, dz: float, interbin=False) -> np.ndarray:
     """Whole plane, K rows ascending in z (reading R9).  For sizes that fit in memory."""
     zs = bank_z(zmax, dz)
     return np.stack([plane_row(spectrum, z, interbin) for z in zs])
 
 
-def plane_cells(spectrum, z: float, cols, interbin: bool = False) -> np.ndarray:
+def plane_cells(spectrum, z: float, cols, interbin=False) -> np.ndarray:
     """
     Sampled cells of one row.  `cols` are plane column indices (0..N-1, or 0..2N-1 when
     interbinned: even 2r -> bin r, odd 2r+1 -> bin r+1/2).
     """
     a = _as_c64(spectrum)
-    h = taps(z)
     cols = np.asarray(cols, dtype=np.int64)
+    if int(interbin) == 2:
+        return power_from_amplitudes(correlate_at(interleave_zeros(a), taps2(z), cols))
+    h = taps(z)
     if not interbin:
         return power_from_amplitudes(correlate_at(a, h, cols))
     r = cols // 2
@@ -230,7 +261,7 @@ def plane_cells(spectrum, z: float, cols, interbin: bool = False) -> np.ndarray:
                     power_from_amplitudes(y0))
 
 
-def candidates(spectrum, zmax: float, dz: float, threshold: float, interbin: bool = False):
+def candidates(spectrum, zmax: float, dz: float, threshold: float, interbin=False):
     """
     Threshold search of the plane ("calculating the power spectrum, and comparing the
     resulting Fourier power to a pre-calculated threshold"; PAPER.md:331 names search / candidate

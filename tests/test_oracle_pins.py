@@ -331,3 +331,56 @@ def test_p11_injected_chirp_is_the_candidate():
     rows, cols, pows = orc.candidates(b, 4.0, 2.0, 0.9 * amp ** 2, True)
     i = int(np.argmax(pows))
     assert (rows[i], cols[i]) == (2, 2 * r0 + 1)
+
+
+# ---------------------------------------------------------------- P12: 2-bin Fourier interpolation (R16)
+def test_p12_half_offset_response_is_the_dft_of_a_half_bin_chirp():
+    # time-domain chirp centred on a half-integer frequency, DFT at integer bins k: h_z(k - r_c) with
+    # k - r_c half-integer.  Endpoint (Riemann) term makes this O(1/Nt) for fractional r_c.
+    nt, rc, z = 8192, 700.5, 12.0
+    u = np.arange(nt) / nt
+    x = np.exp(2j * np.pi * (rc * u + z * (u * u - u) / 2.0))
+    spec = np.fft.fft(x) / nt
+    m = orc.halfwidth(z)
+    t2 = orc.taps2(z)                                   # h_z(j/2), j = -2m..2m
+    odd = t2[1::2]                                      # j = -2m+1, -2m+3, ...: offsets d - 1/2, d = -m+1..m
+    k = np.arange(-m + 1, m + 1) + int(rc - 0.5)        # k - rc = d - 1/2
+    assert np.max(np.abs(spec[k] - odd)) < 3.0 / nt
+    assert np.allclose(t2[0::2], orc.taps(z), rtol=0, atol=1e-15)         # even j: the integer-offset taps
+    assert np.max(np.abs(odd + odd[::-1])) < 1e-14                        # h(x) = -h(-x) at half-integers
+
+
+def test_p12_even_columns_are_the_plain_plane_and_z0_is_zero_padded_dft():
+    nt = 4096
+    rng = np.random.default_rng(5)
+    x = rng.standard_normal(nt) + 1j * rng.standard_normal(nt)
+    a = (np.fft.fft(x) / nt).astype(np.complex64)
+    for z in (0.0, 6.0, -20.0):
+        p2 = orc.plane_row(a, z, 2)
+        assert p2.size == 2 * nt
+        assert np.allclose(p2[0::2], orc.plane_row(a, z, 0), rtol=1e-12, atol=0)
+    # z = 0: the half-bin amplitudes are the DFT of the time series zero-padded to 2 Nt (exact Fourier
+    # interpolation) up to the truncation of the sinc taps, which shrinks as the half-width grows
+    x64 = np.fft.ifft(a.astype(np.complex128)) * nt
+    fine = np.abs(np.fft.fft(np.concatenate([x64, np.zeros(nt)])) / nt) ** 2
+    errs = []
+    for m in (16, 128, 1024):
+        p2 = orc.plane_row(a, 0.0, 2, m=m)
+        sl = slice(2 * m + 1, 2 * (nt - m) - 1, 2)      # odd columns away from the zero-extended edges
+        errs.append(np.sqrt(np.mean((p2[sl] - fine[sl]) ** 2)) / np.mean(fine[sl]))
+    assert errs[0] > errs[1] > errs[2] and errs[2] < 2e-2, errs
+
+
+def test_p12_half_bin_chirp_peaks_in_its_odd_column():
+    n, r0, z0, amp = 1 << 13, 3000, 8.0, 5.0
+    a = syn.chirp_spectrum(n, [(r0 + 0.5, z0, amp)]).astype(np.complex64)
+    zs = orc.bank_z(20.0, 2.0)
+    pl = np.stack([orc.plane_row(a, z, 2) for z in zs])
+    k, c = np.unravel_index(np.argmax(pl), pl.shape)
+    assert zs[k] == z0 and c == 2 * r0 + 1
+    e = np.sum(np.abs(orc.taps2(z0)[1::2]) ** 2)        # energy of the truncated half-offset taps
+    assert abs(pl[k, c] - amp ** 2 * e ** 2) < 1e-3 * amp ** 2 and 0.95 < e < 1.0
+    # unit white noise: odd columns average to that energy (as P8)
+    b = syn.make_spectrum(1 << 16, 34)
+    p = orc.plane_row(b, z0, 2)
+    assert abs(np.mean(p[1::2]) - e) < 12.0 / math.sqrt(b.size)

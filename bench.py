@@ -158,14 +158,19 @@ class CufftUnfused:
         info = plan.info
         self.N, self.K, self.L = int(info.nbins), int(info.ntemplates), int(info.seglen)
         self.ov, self.B, self.nseg = int(info.overlap), int(info.useful), int(info.nseg)
-        self.interbin = bool(info.interbin)
-        g = np.zeros((self.K, self.L), dtype=np.complex128)
-        for k in range(self.K):
-            h = fdas.fdas_get_taps(plan.handle, k)           # h[d + m_k], d = -m_k..m_k
-            mk = (h.size - 1) // 2
-            d = np.arange(-mk, mk + 1)
-            g[k, (-d) % self.L] = np.conj(h)                  # correlation as circular convolution
-        self.H = torch.from_numpy((np.fft.fft(g, axis=1) / self.L).astype(np.complex64)).to(dev)
+        self.interbin = int(info.interbin)
+
+        def bank(first):
+            g = np.zeros((self.K, self.L), dtype=np.complex128)
+            for k in range(self.K):
+                h = fdas.fdas_get_taps(plan.handle, first + k)   # h[d + m_k], d = -m_k..m_k
+                mk = (h.size - 1) // 2
+                d = np.arange(-mk, mk + 1)
+                g[k, (-d) % self.L] = np.conj(h)              # correlation as circular convolution
+            return torch.from_numpy((np.fft.fft(g, axis=1) / self.L).astype(np.complex64)).to(dev)
+
+        self.H = bank(0)
+        self.H2 = bank(self.K) if self.interbin == 2 else None   # two-bin interpolation: taps h_z(d - 1/2)
         self.padded = torch.zeros(self.ov + self.nseg * self.B + self.L, dtype=torch.complex64, device=dev)
 
     def run(self, d_spec, d_plane):
@@ -177,7 +182,14 @@ class CufftUnfused:
         Y = X.unsqueeze(0) * self.H.unsqueeze(1)                             # step 3: K x nseg x L products
         y = torch.fft.ifft(Y, dim=2, norm="forward")                         # step 4: cuFFT inverse (1/L in H)
         del Y
-        if not self.interbin:                                                # step 5: discard + power
+        if self.interbin == 2:                       # odd columns from the half-bin bank, even from the plain one
+            y2 = torch.fft.ifft(X.unsqueeze(0) * self.H2.unsqueeze(1), dim=2, norm="forward")
+            out = torch.empty((K, nseg * B, 2), dtype=torch.float32, device=d_plane.device)
+            for j, yy in enumerate((y, y2)):
+                v = torch.view_as_real(yy[:, :, ov:ov + B])
+                out[:, :, j] = (v[..., 0] ** 2 + v[..., 1] ** 2).reshape(K, nseg * B)
+            d_plane.copy_(out[:, :N].reshape(K, 2 * N))
+        elif not self.interbin:                                              # step 5: discard + power
             yv = torch.view_as_real(y[:, :, ov:ov + B])
             P = (yv[..., 0] ** 2 + yv[..., 1] ** 2).reshape(K, nseg * B)
             d_plane.copy_(P[:, :N])

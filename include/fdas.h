@@ -14,6 +14,9 @@
  *       FFT, inverse FFT, discard the contaminated edges, power, contiguous store.
  *   interbinning (PAPER.md:81-83 eq. 4, :89, :95), applied to the correlated amplitudes:
  *       P[z][2r] = |y_z[r]|^2,  P[z][2r+1] = |(pi/4)(y_z[r] - y_z[r+1])|^2
+ *   two-bin Fourier interpolation ("doubling the template and signal resolution using
+ *   interleaving zeros prior to the correlations"; reading R16), the accurate alternative:
+ *       P[z][2r] = |y_z[r]|^2,  P[z][2r+1] = |sum_{d=-m_z+1}^{m_z} A[r+d] * conj(h_z(d - 1/2))|^2
  *
  * All entry points are plain C, take plain pointers and sizes, return a status code and
  * never throw or abort.  "device" pointers are CUDA device pointers on the device that
@@ -56,7 +59,7 @@ typedef struct fdas_info {
     int32_t overlap;      /* bins discarded at each end of a segment (>= m, +1 with interbinning;
                              rounded up to a multiple of 32 so segment loads/stores stay 128B-aligned) */
     int32_t useful;       /* B = L - 2*overlap useful output bins per segment                        */
-    int32_t interbin;     /* 0/1                                                                     */
+    int32_t interbin;     /* 0 none, 1 interbinning (eq. 4), 2 two-bin Fourier interpolation         */
     int32_t npairs;       /* (K+1)/2 template slots processed by the kernel (+-z share one slot)      */
     int32_t threads;      /* threads per CTA of the fused kernel                                     */
     int32_t grid;         /* CTAs launched by fdas_execute (persistent; multiple of the SM count)    */
@@ -71,7 +74,10 @@ typedef struct fdas_info {
  * Create a plan for spectra of `nbins` complex64 bins and the template bank
  * z = -zmax .. +zmax step dz ("K acceleration templates"; BASELINE.json),
  * each template of half-width ceil(|z|/2)+16 bins (R4), segment FFT length `seglen`
- * ("blocks of length L"), with or without interbinning.
+ * ("blocks of length L"); `interbin` = 0: N columns; 1: 2N columns, half-bin cells
+ * by interbinning (eq. 4), any seglen; 2: 2N columns, half-bin cells by two-bin
+ * Fourier interpolation (a second template bank, twice the transforms;
+ * seglen <= 4096, FDAS_ERR_UNSUPPORTED at 8192).
  * Allocates the plan-owned device memory (taps, template spectra, twiddle table).
  * *out is set to NULL on failure.
  */
@@ -157,6 +163,8 @@ fdas_status fdas_plan_info(const fdas_plan *plan, fdas_info *out);
  * Copy template k's taps to the host (synchronises): host_re_im receives
  * 2*(2*halfwidth_k+1) doubles, interleaved (re, im), index d + halfwidth_k <-> tap d.
  * The buffer must hold 2*(2*info.halfwidth+1) doubles.  Needs fdas_make_templates.
+ * With interbin = 2, k in [ntemplates, 2*ntemplates) addresses the half-bin bank of template
+ * k - ntemplates: index d + halfwidth_k <-> h_z(d - 1/2), d = -halfwidth_k+1..halfwidth_k (index 0 is 0).
  */
 fdas_status fdas_get_taps(fdas_plan *plan, int32_t k, double *host_re_im, int32_t *halfwidth_k);
 

@@ -21,6 +21,7 @@ struct fdas_plan {
     fdas_info info;
     int device;
     bool ready;
+    int nbanks;          // 2 with two-bin Fourier interpolation (bank 1: half-bin templates)
     double2 *d_taps;     // K x (2m+1)
     float2 *d_hperm;     // npairs x L (kernel register order)
     float2 *d_wtab;      // L (seglen 8192: the 4096 table)
@@ -51,8 +52,9 @@ namespace {
 typedef void (*kernel_fn)(const KernelParams);
 
 template <int L, int MINB>
-kernel_fn pick_kernel(bool ib, int mode)
+kernel_fn pick_kernel(int ib, int mode)
 {
+    if (ib == 2) return mode ? (kernel_fn)fdas_fused_kernel<L, false, MINB, 1, 2> : (kernel_fn)fdas_fused_kernel<L, false, MINB, 0, 2>;
     if (mode) return ib ? (kernel_fn)fdas_fused_kernel<L, true, MINB, 1> : (kernel_fn)fdas_fused_kernel<L, false, MINB, 1>;
     return ib ? (kernel_fn)fdas_fused_kernel<L, true, MINB> : (kernel_fn)fdas_fused_kernel<L, false, MINB>;
 }
@@ -60,20 +62,23 @@ kernel_fn pick_kernel(bool ib, int mode)
 // L = 4096: second-generation kernel (shuffle exchange, fdas_kernel2.cuh); measured on B200 it is
 // 4.5 % faster than the first at L = 4096 and 7 % slower at L = 2048, which stays on the first.
 template <int L, int MINB>
-kernel_fn pick_kernel2(bool ib, int mode)
+kernel_fn pick_kernel2(int ib, int mode)
 {
+    if (ib == 2) return mode ? (kernel_fn)fdas_fused_kernel2<L, false, MINB, 1, 2> : (kernel_fn)fdas_fused_kernel2<L, false, MINB, 0, 2>;
     if (mode) return ib ? (kernel_fn)fdas_fused_kernel2<L, true, MINB, 1> : (kernel_fn)fdas_fused_kernel2<L, false, MINB, 1>;
     return ib ? (kernel_fn)fdas_fused_kernel2<L, true, MINB> : (kernel_fn)fdas_fused_kernel2<L, false, MINB>;
 }
 
 // mode 0: plane store (fdas_execute); mode 1: threshold search (fdas_execute_threshold)
-kernel_fn select_kernel(int L, bool ib, int mode = 0)
+// ib: 0 none, 1 interbinning (eq. 4), 2 two-bin Fourier interpolation (second template bank; L <= 4096)
+kernel_fn select_kernel(int L, int ib, int mode = 0)
 {
     switch (L) {
     case 1024: return pick_kernel<1024, 4>(ib, mode);
     case 2048: return pick_kernel<2048, 2>(ib, mode);
     case 4096: return pick_kernel2<4096, 1>(ib, mode);
     case 8192:                                                            // 2 x 4096 (fdas_kernel8k.cuh)
+        if (ib == 2) return nullptr;
         if (ib) return mode ? (kernel_fn)fdas_fused_kernel_8k<1, 1, true> : (kernel_fn)fdas_fused_kernel_8k<1, 0, true>;
         return mode ? (kernel_fn)fdas_fused_kernel_8k<1, 1> : (kernel_fn)fdas_fused_kernel_8k<1>;
     default: return nullptr;
@@ -132,23 +137,24 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double
     const double nh = zmax / dz;
     const double nhr = std::floor(nh + 0.5);
     if (std::fabs(nh - nhr) > 1e-9 * std::fmax(1.0, nh) || nhr > 1e6) return FDAS_ERR_INVALID_ARG;
-    if (interbin != 0 && interbin != 1) return FDAS_ERR_INVALID_ARG;
+    if (interbin < 0 || interbin > 2) return FDAS_ERR_INVALID_ARG;
     if (seglen != 1024 && seglen != 2048 && seglen != 4096 && seglen != 8192)
         return FDAS_ERR_UNSUPPORTED;
 
     const int K = 2 * (int)nhr + 1;
     const int m = (int)std::ceil(zmax * 0.5 - 1e-12) + 16;
-    const int ov = ((m + interbin) + 31) / 32 * 32; // >= m (+1 for the interbin neighbour), 128B-aligned
+    const int ov = ((m + (interbin ? 1 : 0)) + 31) / 32 * 32; // >= m (+1 for the interbin neighbour), 128B-aligned
     const int B = seglen - 2 * ov;
     if (B < 32) return FDAS_ERR_UNSUPPORTED;
-    kernel_fn kern = select_kernel(seglen, interbin != 0);
+    kernel_fn kern = select_kernel(seglen, interbin);
     if (!kern) return FDAS_ERR_UNSUPPORTED;
 
     fdas_plan *p = new (std::nothrow) fdas_plan();
     if (!p) return FDAS_ERR_NOMEM;
     std::memset(p, 0, sizeof(*p));
     p->kernel = kern;
-    p->kernel_thr = select_kernel(seglen, interbin != 0, 1);
+    p->kernel_thr = select_kernel(seglen, interbin, 1);
+    p->nbanks = interbin == 2 ? 2 : 1;
     fdas_info &I = p->info;
     I.nbins = nbins;
     I.ncols = interbin ? 2 * nbins : nbins;
@@ -165,7 +171,7 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double
     I.interbin = interbin;
     I.npairs = (K + 1) / 2;
     I.threads = seglen == 8192 ? 256 : seglen / 16;
-    I.smem_bytes = smem_bytes_for(seglen, interbin != 0);
+    I.smem_bytes = smem_bytes_for(seglen, interbin == 1);
 
     fdas_status st = FDAS_OK;
     do {
@@ -190,8 +196,8 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double
 #endif
         I.ctas_per_sm = occ;
         I.grid = occ * I.sm_count;
-        const size_t taps_bytes = (size_t)K * (2 * m + 1) * sizeof(double2);
-        const size_t h_bytes = (size_t)I.npairs * seglen * sizeof(float2);
+        const size_t taps_bytes = (size_t)p->nbanks * K * (2 * m + 1) * sizeof(double2);
+        const size_t h_bytes = (size_t)p->nbanks * I.npairs * seglen * sizeof(float2);
         if (cudaMalloc(&p->d_taps, taps_bytes) != cudaSuccess ||
             cudaMalloc(&p->d_hperm, h_bytes) != cudaSuccess ||
             cudaMalloc(&p->d_wtab, (size_t)seglen * sizeof(float2)) != cudaSuccess ||
@@ -217,7 +223,10 @@ fdas_status fdas_make_templates(fdas_plan *p, void *stream)
     const int w = 2 * I.halfwidth + 1;
     {
         const int n = I.ntemplates * w;
-        make_taps_kernel<<<(n + 127) / 128, 128, 0, st>>>(p->d_taps, I.ntemplates, I.halfwidth, I.zmax, I.dz);
+        for (int b = 0; b < p->nbanks; ++b)
+            make_taps_kernel<<<(n + 127) / 128, 128, 0, st>>>(p->d_taps + (size_t)b * n, I.ntemplates, I.halfwidth,
+                                                              I.zmax, I.dz, b);
+        g_launches += p->nbanks - 1;
         const int lw = I.seglen == 8192 ? 4096 : I.seglen;   // table of the kernel's passes
         make_wtab_kernel<<<(lw + 127) / 128, 128, 0, st>>>(p->d_wtab, lw);
         if (I.seglen == 8192) {
@@ -227,9 +236,21 @@ fdas_status fdas_make_templates(fdas_plan *p, void *stream)
         const int nh = I.npairs * I.seglen;
         const int gb = (nh + 127) / 128;
         switch (I.seglen) {
-        case 1024: make_spectra_kernel<1024><<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps, I.npairs, I.halfwidth, I.zmax, I.dz, I.ntemplates); break;
-        case 2048: make_spectra_kernel<2048><<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps, I.npairs, I.halfwidth, I.zmax, I.dz, I.ntemplates); break;
-        case 4096: make_spectra_kernel<4096><<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps, I.npairs, I.halfwidth, I.zmax, I.dz, I.ntemplates); break;
+        case 1024:
+            for (int b = 0; b < p->nbanks; ++b)
+                make_spectra_kernel<1024><<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps + (size_t)b * n, I.npairs, I.halfwidth,
+                                                            I.zmax, I.dz, I.ntemplates, p->nbanks, b);
+            break;
+        case 2048:
+            for (int b = 0; b < p->nbanks; ++b)
+                make_spectra_kernel<2048><<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps + (size_t)b * n, I.npairs, I.halfwidth,
+                                                            I.zmax, I.dz, I.ntemplates, p->nbanks, b);
+            break;
+        case 4096:
+            for (int b = 0; b < p->nbanks; ++b)
+                make_spectra_kernel<4096><<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps + (size_t)b * n, I.npairs, I.halfwidth,
+                                                            I.zmax, I.dz, I.ntemplates, p->nbanks, b);
+            break;
         case 8192: make_spectra_kernel_8k<<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps, I.npairs, I.halfwidth, I.zmax, I.dz, I.ntemplates); break;
         default: return FDAS_ERR_UNSUPPORTED;
         }
@@ -259,7 +280,7 @@ static fdas_status launch_fused(fdas_plan *p, void *stream, const void *d_spectr
     prm.ncols = I.ncols;
     prm.nseg = I.nseg;
     prm.ntemplates = I.ntemplates;
-    prm.npairs = I.npairs;
+    prm.npairs = I.npairs * p->nbanks;      // template slots per segment (bank-minor)
     prm.overlap = I.overlap;
     prm.useful = I.useful;
     void *args[] = {&prm};
@@ -382,12 +403,13 @@ fdas_status fdas_plan_info(const fdas_plan *p, fdas_info *out)
 
 fdas_status fdas_get_taps(fdas_plan *p, int32_t k, double *host_re_im, int32_t *halfwidth_k)
 {
-    if (!p || !host_re_im || !halfwidth_k || k < 0 || k >= p->info.ntemplates) return FDAS_ERR_INVALID_ARG;
+    if (!p || !host_re_im || !halfwidth_k || k < 0 || k >= p->info.ntemplates * p->nbanks) return FDAS_ERR_INVALID_ARG;
     if (!p->ready) return FDAS_ERR_NOT_READY;
     const fdas_info &I = p->info;
     const int m = I.halfwidth, w = 2 * m + 1;
+    const int kk = k % I.ntemplates;            // k >= ntemplates: bank 1 (interbin = 2), taps h_z(d - 1/2)
     const int center = (I.ntemplates - 1) / 2;
-    const double z = (k == center) ? 0.0 : -I.zmax + k * I.dz;
+    const double z = (kk == center) ? 0.0 : -I.zmax + kk * I.dz;
     const int mz = (int)std::ceil(std::fabs(z) * 0.5 - 1e-12) + 16;
     FDAS_CUDA(p, cudaDeviceSynchronize());
     FDAS_CUDA(p, cudaMemcpy(host_re_im, p->d_taps + (size_t)k * w + (m - mz),
@@ -406,7 +428,7 @@ fdas_status fdas_get_template_spectrum(fdas_plan *p, int32_t k, float *host_re_i
     const bool conj = k != pair;
     std::vector<float2> buf(L);
     FDAS_CUDA(p, cudaDeviceSynchronize());
-    FDAS_CUDA(p, cudaMemcpy(buf.data(), p->d_hperm + (size_t)pair * L, (size_t)L * sizeof(float2),
+    FDAS_CUDA(p, cudaMemcpy(buf.data(), p->d_hperm + (size_t)pair * p->nbanks * L, (size_t)L * sizeof(float2),
                             cudaMemcpyDeviceToHost));
     for (int f = 0; f < L; ++f) {
         int tid, i;

@@ -470,7 +470,12 @@ __device__ __forceinline__ void flush_edges(const KernelParams &prm, const Threa
 // Persistent fused kernel.  Work = nseg * npairs (segment, template-slot) units, split into
 // gridDim.x equal contiguous ranges (segment-major), so each CTA redoes at most one extra
 // forward FFT at a range boundary and every CTA gets the same number of inverse FFT pairs.
-template <int L, bool INTERBIN, int MINB, int MODE = 0>
+// BANKS = 2 (two-bin Fourier interpolation, reading R16): prm.npairs counts template SLOTS,
+// slot = 2 * pair + bank; bank 0 holds the usual templates and fills the even plane columns, bank 1 the
+// templates sampled at half-integer offsets t[d] = h_z(d - 1/2) and fills the odd columns.  The +-z pairing
+// survives with a one-bin shift: conj(H_bank1 of -|z|) = exp(-2 pi i f / L) H_bank1 of +|z| (h is odd about
+// 1/2 there), so the q transform's output n is the half-bin cell of bin n - 1.
+template <int L, bool INTERBIN, int MINB, int MODE = 0, int BANKS = 1>
 __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const KernelParams prm)
 {
     using G = Geo<L>;
@@ -520,6 +525,14 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
         if (nn >= prm.overlap && nn < prm.overlap + prm.useful) vmask |= 1u << n1;
     }
 
+    unsigned vmask_q1 = 0;                       // BANKS = 2, bank 1, q row: output n is bin n - 1
+    if constexpr (BANKS == 2) {
+#pragma unroll
+        for (int n1 = 0; n1 < 16; ++n1) {
+            const int nn = n1 * G::Q + tid - 1;
+            if (nn >= prm.overlap && nn < prm.overlap + prm.useful) vmask_q1 |= 1u << n1;
+        }
+    }
     Pending<L> pend{0, 0, 0, false};
     bool have_q3 = false;
 
@@ -554,24 +567,33 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
 
         if (INTERBIN && pend.on) flush_edges<L, MODE>(prm, tm, edges, pend);   // every warp is past Q1(c-1)
 
-        const int row_p = pair;                         // z <= 0
-        const int row_q = prm.ntemplates - 1 - pair;    // z >= 0 (same row for the z = 0 slot)
+        const int bank = BANKS == 2 ? (pair & 1) : 0;
+        const int row_p = BANKS == 2 ? (pair >> 1) : pair;   // z <= 0
+        const int row_q = prm.ntemplates - 1 - row_p;   // z >= 0 (same row for the z = 0 slot)
         const long long col0 = seg * prm.useful - prm.overlap;  // column of local index 0
         cpk y[16];
         inv_q1<L>(tm, e1, y);
         unsigned vm = vmask;
-        if (col0 + prm.overlap + prm.useful > prm.nbins) {
+        unsigned vmq = bank ? vmask_q1 : vmask;
+        if (col0 + prm.overlap + prm.useful >= prm.nbins) {
 #pragma unroll
-            for (int n1 = 0; n1 < 16; ++n1)
+            for (int n1 = 0; n1 < 16; ++n1) {
                 if (col0 + n1 * G::Q + tid >= prm.nbins) vm &= ~(1u << n1);
+                if (col0 + n1 * G::Q + tid - bank >= prm.nbins) vmq &= ~(1u << n1);
+            }
         }
         // The z = 0 slot has row_q == row_p and q == p bit for bit (H_0 is real), so its second
         // store rewrites the same value: no special case (MODE 1 reports the cell once: vq = 0).
         const unsigned qon = (MODE != 0 && row_q == row_p) ? 0u : ~0u;
-        if constexpr (!INTERBIN) {
+        if constexpr (BANKS == 2) {
+            // column 2 * bin + bank; the z = 0 slot's q row is its p row again (one bin off in bank 1): skipped
+            float *bp = prm.plane + (size_t)row_p * prm.ncols + (2 * (col0 + tid) + bank);
+            float *bq = prm.plane + (size_t)row_q * prm.ncols + (2 * (col0 + tid - bank) + bank);
+            emit_unit<L, false, MODE, 2>(prm, y, bp, bq, vm, row_q == row_p ? 0u : vmq);
+        } else if constexpr (!INTERBIN) {
             float *bp = prm.plane + (size_t)row_p * prm.ncols + (col0 + tid);
             float *bq = prm.plane + (size_t)row_q * prm.ncols + (col0 + tid);
-            emit_unit<L, false, MODE, 1>(prm, y, bp, bq, vm, vm & qon);
+            emit_unit<L, false, MODE, 1>(prm, y, bp, bq, vm, vmq & qon);
         } else {
             // lanes 0 and 31 post their y to the mailbox; lane 31's cells (power and half-bin) are
             // written one unit later by flush_edges, every other lane stores (P[n], P[n+1/2]) now
@@ -586,7 +608,7 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel(const Kerne
             if (tm.lane == 31) vm = 0;
             emit_unit<L, true, MODE, 1>(prm, y, bp, bq, vm, vm & qon);
             pend.col0 = col0;
-            pend.pair = pair;
+            pend.pair = row_p;
             pend.par = par;
             pend.on = true;
         }

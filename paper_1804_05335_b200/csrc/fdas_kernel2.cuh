@@ -190,7 +190,7 @@ __device__ __forceinline__ void inv_q3_q2(const float2 (&xh)[Geo<L>::PTS], const
     q3_tail_q2<L>(a, tw, tm, out);
 }
 
-template <int L, bool INTERBIN, int MINB, int MODE = 0>
+template <int L, bool INTERBIN, int MINB, int MODE = 0, int BANKS = 1>   // BANKS = 2: see fdas_kernel.cuh
 __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const KernelParams prm)
 {
     using G = Geo<L>;
@@ -240,6 +240,14 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
         if (nn >= prm.overlap && nn < prm.overlap + prm.useful) vmask |= 1u << n1;
     }
 
+    unsigned vmask_q1 = 0;                       // BANKS = 2, bank 1, q row: output n is bin n - 1
+    if constexpr (BANKS == 2) {
+#pragma unroll
+        for (int n1 = 0; n1 < 16; ++n1) {
+            const int nn = n1 * G::Q + tid - 1;
+            if (nn >= prm.overlap && nn < prm.overlap + prm.useful) vmask_q1 |= 1u << n1;
+        }
+    }
     Pending<L> pend[2] = {{0, 0, 0, false}, {0, 0, 1, false}};
     auto e1buf = [&](int u) {
         float2 *b = e1base + (u & 1) * 2 * G::E1_ELEMS;
@@ -262,8 +270,9 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
     auto consume = [&](int q, int qpair) {
         mbar_wait(&full[q & 1], (q >> 1) & 1);                 // all of E1[q & 1] is written
         const XBuf e1 = e1buf(q);
-        const int row_p = qpair;                        // z <= 0
-        const int row_q = prm.ntemplates - 1 - qpair;   // z >= 0 (same row for the z = 0 slot)
+        const int bank = BANKS == 2 ? (qpair & 1) : 0;
+        const int row_p = BANKS == 2 ? (qpair >> 1) : qpair;   // z <= 0
+        const int row_q = prm.ntemplates - 1 - row_p;   // z >= 0 (same row for the z = 0 slot)
         const long long col0 = seg * prm.useful - prm.overlap;  // column of local index 0
         const unsigned qon = (MODE != 0 && row_q == row_p) ? 0u : ~0u;   // MODE 1: z = 0 cell reported once
         cpk y[16];
@@ -273,15 +282,22 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
         dft<+1, 16>(y);
         // columns >= nbins (last segment): outputs n1 >= ceil((nbins - col0 - tid) / Q) are dropped
         unsigned vm = vmask;
-        if (col0 + prm.overlap + prm.useful > prm.nbins) {
+        unsigned vmq = bank ? vmask_q1 : vmask;
+        if (col0 + prm.overlap + prm.useful >= prm.nbins) {
 #pragma unroll
-            for (int n1 = 0; n1 < 16; ++n1)
+            for (int n1 = 0; n1 < 16; ++n1) {
                 if (col0 + n1 * G::Q + tid >= prm.nbins) vm &= ~(1u << n1);
+                if (col0 + n1 * G::Q + tid - bank >= prm.nbins) vmq &= ~(1u << n1);
+            }
         }
-        if constexpr (!INTERBIN) {
+        if constexpr (BANKS == 2) {
+            float *bp = prm.plane + (size_t)row_p * prm.ncols + (2 * (col0 + tid) + bank);
+            float *bq = prm.plane + (size_t)row_q * prm.ncols + (2 * (col0 + tid - bank) + bank);
+            emit_unit<L, false, MODE, 2>(prm, y, bp, bq, vm, row_q == row_p ? 0u : vmq);
+        } else if constexpr (!INTERBIN) {
             float *bp = prm.plane + (size_t)row_p * prm.ncols + (col0 + tid);
             float *bq = prm.plane + (size_t)row_q * prm.ncols + (col0 + tid);
-            emit_unit<L, false, MODE, 1>(prm, y, bp, bq, vm, vm & qon);
+            emit_unit<L, false, MODE, 1>(prm, y, bp, bq, vm, vmq & qon);
         } else {
             const int par = q & 1;
             float4 *eb = edges + par * (2 * G::W * 16) + (tm.lane == 0 ? G::W * 16 : 0) + tm.warp * 16;
@@ -296,7 +312,7 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
             if (tm.lane == 31) vm = 0;
             emit_unit<L, true, MODE, 1>(prm, y, bp, bq, vm, vm & qon);
             pend[par].col0 = col0;
-            pend[par].pair = qpair;
+            pend[par].pair = row_p;
             pend[par].par = par;
             pend[par].on = true;
         }

@@ -6,6 +6,8 @@
 //          z > 0, q = -d - z/2, Y = q sqrt(2/z), Z = (q+z) sqrt(2/z):
 //          h_z(d) = exp(-i pi q^2 / z) / sqrt(2 z) * { [C(Z)-C(Y)] + i [S(Z)-S(Y)] }
 //          z < 0: h_z(d) = conj(h_{-z}(-d));   z = 0: Kronecker delta at integer d.
+//      Bank 1 (2-bin Fourier interpolation, reading R16) holds the same response
+//      at the half-integer offsets d - 1/2, d = -m_z+1..m_z (z = 0: exp(-i pi x) sin(pi x)/(pi x)).
 //  a1  spectra: H_z[f] = (1/L) sum_d conj(h_z[d]) exp(+2 pi i d f / L)   (the
 //      filter centred at bin 0, halves at both ends of the L-array; 1/L of eq. 6 folded in, R6),
 //      written in the register order of the fused kernel's un-permuted FFT.
@@ -81,8 +83,9 @@ __device__ inline int tap_halfwidth(double z)
     return (int)ceil(fabs(z) * 0.5 - 1e-12) + 16; // R4: ceil(|z|/2) + 16
 }
 
-// taps[k][d + m], d = -m..m (m = bank half-width); zero for |d| > m_z.
-__global__ void make_taps_kernel(double2 *taps, int K, int m, double zmax, double dz)
+// taps[k][d + m], d = -m..m (m = bank half-width); zero for |d| > m_z.  half = 1: bank 1, the tap at
+// index d is h_z(d - 1/2), d = -m_z+1..m_z.
+__global__ void make_taps_kernel(double2 *taps, int K, int m, double zmax, double dz, int half)
 {
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
     const int w = 2 * m + 1;
@@ -92,13 +95,21 @@ __global__ void make_taps_kernel(double2 *taps, int K, int m, double zmax, doubl
     const double z = (k == center) ? 0.0 : -zmax + k * dz;
     const int mz = tap_halfwidth(z);
     double2 h = make_double2(0.0, 0.0);
-    if (d >= -mz && d <= mz) {
+    if (d >= -mz + half && d <= mz) {
+        const double x = (double)d - 0.5 * half;
         if (z == 0.0) {
-            h.x = (d == 0) ? 1.0 : 0.0;
+            if (half) {                                  // exp(-i pi x) sinc(x) at half-integer x
+                double sn, cs;
+                sincospi(x, &sn, &cs);
+                const double sc = sn / (3.14159265358979323846264338327950288 * x);
+                h = make_double2(cs * sc, -sn * sc);
+            } else {
+                h.x = (d == 0) ? 1.0 : 0.0;
+            }
         } else if (z > 0.0) {
-            h = response_closed_form(z, (double)d);
+            h = response_closed_form(z, x);
         } else {
-            h = response_closed_form(-z, (double)(-d));
+            h = response_closed_form(-z, -x);
             h.y = -h.y;
         }
     }
@@ -115,9 +126,10 @@ __global__ void make_wtab_kernel(float2 *wtab, int L)
 }
 
 // hperm[pair][i/2][tid] (float4 = two complex) for the rows z <= 0 (pair = row index k).
+// nbanks = 2: slot = pair * 2 + bank; `taps` points at the bank's tap array.
 template <int L>
 __global__ void make_spectra_kernel(float2 *hperm, const double2 *taps, int npairs, int m,
-                                    double zmax, double dz, int K)
+                                    double zmax, double dz, int K, int nbanks, int bank)
 {
     using G = Geo<L>;
     const int idx = blockIdx.x * blockDim.x + threadIdx.x;
@@ -139,7 +151,7 @@ __global__ void make_spectra_kernel(float2 *hperm, const double2 *taps, int npai
     }
     int tid, i;
     freq_to_reg<L>(f, tid, i);
-    const size_t off = (((size_t)pair * (G::PTS / 2) + (i >> 1)) * G::T + tid) * 2 + (i & 1);
+    const size_t off = ((((size_t)pair * nbanks + bank) * (G::PTS / 2) + (i >> 1)) * G::T + tid) * 2 + (i & 1);
     hperm[off] = make_float2((float)(sr / L), (float)(si / L));
 }
 

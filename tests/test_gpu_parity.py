@@ -58,7 +58,7 @@ def check_rows(orc, spectrum, plane, zmax, dz, interbin, rows=None):
     zs = orc.bank_z(zmax, dz)
     worst_max, worst_l2 = 0.0, 0.0
     for k in (range(zs.size) if rows is None else rows):
-        ref = orc.plane_row(spectrum, zs[k], bool(interbin))
+        ref = orc.plane_row(spectrum, zs[k], int(interbin))
         got = plane[k].astype(np.float64)
         assert got.shape == ref.shape
         assert np.all(np.isfinite(got)), f"row {k}: unwritten or non-finite cells"
@@ -196,6 +196,39 @@ def test_seglen_8192_interbin(torch, fd, orc, syn, nbins, zmax):
     plane, info = run_gpu(torch, fd, spec, zmax, 4.0, 8192, 1)
     assert plane.shape == (info["ntemplates"], 2 * nbins) and info["overlap"] >= info["halfwidth"] + 1
     check_rows(orc, spec, plane, zmax, 4.0, 1)
+
+
+@pytest.mark.parametrize("nbins,zmax,seglen", [(1 << 15, 20.0, 1024), (50021, 84.0, 2048), (1 << 16, 84.0, 4096),
+                                               (3, 20.0, 1024), (1921, 84.0, 2048)])
+def test_two_bin_fourier_interpolation(torch, fd, orc, syn, nbins, zmax, seglen):
+    """interbin = 2 (reading R16): even columns = the plain plane, odd columns = the correlation
+    with the templates at half-integer offsets (second template bank); against the oracle's zero-interleaved
+    double-resolution correlation.  Chirps sit on half bins, at z = 0 and at the right edge."""
+    chirps = ([(int(0.3 * nbins) + 0.5, 0.5 * zmax, 30.0), (int(0.6 * nbins) + 0.5, 0.0, 15.0), (nbins - 1.5, -zmax, 25.0)]
+              if nbins > 100 else [])
+    spec = syn.make_spectrum(nbins, 222 + seglen, chirps)
+    plane, info = run_gpu(torch, fd, spec, zmax, 2.0, seglen, 2)
+    assert plane.shape == (info["ntemplates"], 2 * nbins) and info["interbin"] == 2
+    check_rows(orc, spec, plane, zmax, 2.0, 2)
+    if nbins > 100:
+        k = int(np.argmax(plane.max(axis=1)))
+        assert plane[k].argmax() % 2 == 1               # the strongest cell is a half-bin cell
+
+
+def test_half_bin_taps_match_oracle_quadrature(torch, fd, orc):
+    """Bank 1 of interbin = 2: Fresnel closed form (and the z = 0 sinc) at half-integer offsets against the
+    oracle's quadrature of the same integral."""
+    for zmax, dz, seglen in [(20.0, 2.0, 1024), (84.0, 2.0, 2048), (6.0, 0.5, 1024)]:
+        with fd.Plan(1 << 14, zmax, dz, seglen, 2) as plan:
+            plan.make_templates()
+            zs = orc.bank_z(zmax, dz)
+            K = zs.size
+            for k, z in enumerate(zs):
+                got = fd.fdas_get_taps(plan.handle, K + k)              # index d + m_z <-> h_z(d - 1/2)
+                ref = orc.taps2(z)[1::2]                                # offsets d - 1/2, d = -m_z+1..m_z
+                assert got.size == 2 * orc.halfwidth(z) + 1 and got[0] == 0
+                assert np.max(np.abs(got[1:] - ref)) < 1e-12, (k, z)
+                assert np.max(np.abs(fd.fdas_get_taps(plan.handle, k) - orc.taps(z))) < 1e-12
 
 
 def test_config5_batch_on_one_stream(torch, fd, orc, syn):

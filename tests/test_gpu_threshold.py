@@ -37,7 +37,7 @@ def check_against_oracle(orc, spec, zmax, dz, interbin, thr, rec):
     key = rec["row"].astype(np.int64) * (1 << 40) + rec["col"]
     assert np.all(np.diff(key) > 0), "a cell was reported twice"
     for k, z in enumerate(zs):
-        ref = orc.plane_row(spec, z, bool(interbin))
+        ref = orc.plane_row(spec, z, int(interbin))
         tol = 1e-4 * ref.max()
         got = rec[rec["row"] == k]
         assert np.all((got["col"] >= 0) & (got["col"] < ref.size))
@@ -57,6 +57,8 @@ def check_against_oracle(orc, spec, zmax, dz, interbin, thr, rec):
     (1 << 17, 84.0, 4096, 1, 10.0),
     (1 << 17, 200.0, 8192, 0, 11.0),
     (1 << 16, 84.0, 8192, 1, 10.0),
+    (1 << 16, 84.0, 2048, 2, 10.0),
+    (40009, 84.0, 4096, 2, 10.0),
 ])
 def test_threshold_candidates_match_oracle(nbins, zmax, seglen, interbin, thr):
     import torch

@@ -44,9 +44,12 @@ NCU_TRAFFIC_BYTES = {2: 671.6e6, 3: 5752.6e6, 4: 7575.0e6, 5: 1395.6e6}
 NCU_TRAFFIC_FILE = {2: "r1c_ncu_config2.md", 3: "r1d_ncu_config3.md", 4: "r1c_ncu_config4.md", 5: "r1c_ncu_config5.md"}
 
 
-def workload(cfg_idx: int):
+def workload(cfg_idx: int, interbin=None):
     from paper_1804_05335_b200 import synthetic
     c = dict(synthetic.CONFIGS[cfg_idx - 1])
+    if interbin is not None and interbin != c["interbin"]:      # --interbin: same spectra, other half-bin mode
+        c["interbin"] = interbin
+        c["name"] += f"+interbin{interbin}"
     K = 2 * int(round(c["zmax"] / c["dz"])) + 1
     m = int(math.ceil(c["zmax"] / 2.0)) + 16
     L = c["seglen"]
@@ -55,9 +58,10 @@ def workload(cfg_idx: int):
     # algorithmic costs per spectrum, SURVEY.md section 8(d) / DESIGN.md "Roofline":
     b_alg = L - 2 * m
     nseg_alg = -(-N // b_alg)
-    flops = nseg_alg * ((1 + K) * 5 * L * math.log2(L) + 6 * K * L + 3 * K * b_alg
-                        + (5 * K * b_alg if c["interbin"] else 0))
-    nbytes = 8 * N + 8 * K * L + 4 * K * ncols
+    nb = 2 if c["interbin"] == 2 else 1           # template banks (two-bin Fourier interpolation: 2)
+    flops = nseg_alg * ((1 + nb * K) * 5 * L * math.log2(L) + 6 * nb * K * L + 3 * nb * K * b_alg
+                        + (5 * K * b_alg if c["interbin"] == 1 else 0))
+    nbytes = 8 * N + 8 * nb * K * L + 4 * K * ncols
     c.update(K=K, m=m, ncols=ncols, cells=K * ncols, alg_flops=flops, alg_bytes=nbytes)
     return c
 
@@ -128,11 +132,11 @@ def cpu_baseline(w, budget_s=15.0):
     zs = orc.bank_z(w["zmax"], w["dz"])
     for z in zs:
         orc.taps(z)                           # templates are excluded from the timed region
-    orc.plane_row(spec[:4096], zs[0], bool(w["interbin"]))     # load the library
+    orc.plane_row(spec[:4096], zs[0], int(w["interbin"]))     # load the library
     t0 = time.perf_counter()
     cells, nrows = 0, 0
     while time.perf_counter() - t0 < budget_s:        # rows 0, 1, 2, ... (wrapping) until the budget is spent
-        p = orc.plane_row(spec, zs[nrows % zs.size], bool(w["interbin"]))
+        p = orc.plane_row(spec, zs[nrows % zs.size], int(w["interbin"]))
         cells += p.size
         nrows += 1
     dt = time.perf_counter() - t0
@@ -235,7 +239,7 @@ def run_reference(args, w):
     def step(i):
         cells = 0
         for k in rng.integers(0, zs.size, rows_per_step):
-            cells += orc.plane_row(spec, zs[k], bool(w["interbin"])).size
+            cells += orc.plane_row(spec, zs[k], int(w["interbin"])).size
         return cells
 
     for i in range(args.warmup):
@@ -263,6 +267,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number 1..5 (default 2: the metric's)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--interbin", type=int, default=None, choices=[0, 1, 2],
+                    help="override the config's half-bin mode (0 none, 1 interbinning, 2 two-bin Fourier interpolation)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cufft", action="store_true",
@@ -272,7 +278,7 @@ def main():
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
-    w = workload(args.config)
+    w = workload(args.config, args.interbin)
     if args.impl == "reference":
         run_reference(args, w)
         return
@@ -411,7 +417,7 @@ def main():
         t_alu = w["alg_flops"] / (fp32_peak * 1e12)
         ach_gbs = w["alg_bytes"] / avg_kernel_s / 1e9
         ach_tf = w["alg_flops"] / avg_kernel_s / 1e12
-        traffic = NCU_TRAFFIC_BYTES.get(args.config)
+        traffic = NCU_TRAFFIC_BYTES.get(args.config) if args.interbin is None else None if args.interbin is None else None
         hbm = {"bound": "hbm", "achieved": ach_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                "frac": ach_gbs / peaks["hbm_gbs"], "traffic": traffic, "peak_source": peaks["source"]}
         alu = {"bound": "alu", "achieved": ach_tf, "peak": fp32_peak, "unit": "TFLOP/s",

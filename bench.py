@@ -260,6 +260,58 @@ def run_reference(args, w):
     }))
 
 
+# Paper's Table 4: independent time series processed in real time on a P100 with the
+# custom-FFT code, sampling interval 64 us.  Rows: n samples -> {K templates: (count without, with interbinning)}.
+# Time per series = n * 64e-6 / count; it INCLUDES the long R2C FFT, which is outside this library's path
+# (BASELINE.md section 2): context, not a target.
+PAPER_TABLE4 = {
+    1 << 20: {64: (41427, 33893), 96: (24900, 19775), 128: (18847, 15277), 192: (12436, 9898), 256: (8039, 6620)},
+    1 << 21: {64: (41645, 34086), 96: (26801, 21123), 128: (20147, 15568), 192: (12216, 9686), 256: (8338, 6757)},
+    1 << 22: {64: (41850, 34322), 96: (27614, 21756), 128: (20455, 16079), 192: (12629, 10043), 256: (8477, 6867)},
+    1 << 23: {64: (42099, 34196), 96: (27826, 21744), 128: (20627, 16199), 192: (12807, 10157), 256: (8600, 6954)},
+}
+
+
+def run_table4():
+    """Table-4-shaped sweep (context): per-series time of fdas_execute for spectra of n/2 bins and K + 1 templates
+    (z = -K..+K step 2; the paper's K is even, this bank is odd), both segment lengths 2048 and 4096, best of the two."""
+    import numpy as np
+    import torch
+    from paper_1804_05335_b200 import fdas, synthetic
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    stream = torch.cuda.Stream(device=dev)
+    rows = []
+    for n, per_k in PAPER_TABLE4.items():
+        N = n // 2
+        spec = torch.from_numpy(synthetic.noise_only_c64(N, 4000 + n % 97).view(np.float32).reshape(N, 2)).to(dev)
+        for K, counts in per_k.items():
+            for ib in (0, 1):
+                best = None
+                for seglen in (2048, 4096):
+                    with fdas.Plan(N, float(K), 2.0, seglen, ib) as plan:
+                        plan.make_templates()
+                        out = torch.empty((plan.info.ntemplates, plan.info.ncols), dtype=torch.float32, device=dev)
+                        evs = [torch.cuda.Event(enable_timing=True) for _ in range(11)]
+                        with torch.cuda.stream(stream):
+                            for _ in range(3):
+                                plan.execute(stream, spec, out)
+                            evs[0].record(stream)
+                            for i in range(10):
+                                plan.execute(stream, spec, out)
+                                evs[i + 1].record(stream)
+                        stream.synchronize()
+                        ms = sorted(evs[i].elapsed_time(evs[i + 1]) for i in range(10))[5]
+                        if best is None or ms < best[0]:
+                            best = (ms, seglen)
+                        del out
+                rows.append({"n_samples": n, "bins": N, "templates": K + 1, "interbin": ib, "seglen": best[1],
+                             "ms": round(best[0], 4),
+                             "paper_p100_ms_incl_r2c_fft": round(n * 64e-6 / counts[ib] * 1e3, 3)})
+    print(json.dumps({"sweep": "paper Table 4 shape (PAPER.md:319, :335-366); this library's time excludes the R2C FFT "
+                               "the paper's includes; other hardware: context, not a target", "rows": rows}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -273,6 +325,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cufft", action="store_true",
                     help="skip the same-box unfused cuFFT comparator (variant A of the paper, N = 1 only)")
+    ap.add_argument("--table4", action="store_true",
+                    help="sweep the shapes of the paper's Table 4 (n = 2^20..2^23 samples, 65..257 templates) and exit")
     ap.add_argument("--probe", action="store_true",
                     help="print the instruction-cost probes (fdas_probe_pipes) as one JSON line and exit")
     args = ap.parse_args()
@@ -287,6 +341,11 @@ def main():
     import torch
     from paper_1804_05335_b200 import dist, fdas, synthetic
 
+    if args.table4:
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py --table4 needs a CUDA device")
+        run_table4()
+        return
     if args.probe:
         if not torch.cuda.is_available():
             raise SystemExit("bench.py --probe needs a CUDA device")

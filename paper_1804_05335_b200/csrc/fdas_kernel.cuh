@@ -414,6 +414,12 @@ __device__ __forceinline__ void emit_unit(const KernelParams &prm, const cpk (&y
     }
 }
 
+__device__ __forceinline__ void st_stream4_if(float *p, float a, float b, float c, float d, unsigned pred)
+{
+    asm volatile("{\n\t.reg .pred pp;\n\tsetp.ne.u32 pp, %5, 0;\n\t@pp st.global.cs.v4.f32 [%0], {%1, %2, %3, %4};\n\t}"
+                 ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d), "r"(pred) : "memory");
+}
+
 // ---- split-phase CTA barrier on shared memory (mbarrier): arrive now, wait later
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t *bar, int count)

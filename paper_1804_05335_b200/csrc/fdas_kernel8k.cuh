@@ -161,6 +161,7 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
     constexpr int SUBS = INTERBIN ? 4 : 2;
     constexpr int CS = INTERBIN ? 2 : 1;              // plane columns per bin
 #define FDAS_Q3_SUB(PAR, HALF) inv_q3_8k<PAR, HALF>(xs_lo, xs_hi, hlo, hhi, wb, tw, tm, e2, prm.wtab2)
+    float2 held[INTERBIN && MODE == 0 ? 48 : 1];      // parked (p, q) powers of sub-units 0..2, see the epilogue
     bool have_q3 = false;
     const int nsub = SUBS * n;
     for (int c = 0; c < nsub; ++c) {
@@ -237,11 +238,47 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
             for (int n1 = 0; n1 < 16; ++n1)
                 if (col0 + 2 * (n1 * G::Q + tid) + par >= prm.nbins) vm &= ~(1u << n1);
         }
-        // bin n = 2n' + par -> plane column CS * (col0 + n) + half
-        float *bp = prm.plane + (size_t)row_p * prm.ncols + (CS * (col0 + 2 * tid + par) + half);
-        float *bq = prm.plane + (size_t)row_q * prm.ncols + (CS * (col0 + 2 * tid + par) + half);
-        const unsigned qon = (MODE != 0 && row_q == row_p) ? 0u : ~0u;   // MODE 1: z = 0 cell reported once
-        emit_unit<4096, false, MODE, 2 * CS>(prm, y, bp, bq, vm, vm & qon);
+        if constexpr (INTERBIN && MODE == 0) {
+            // The four cells of bin pair n' (columns 4n' + {0,1,2,3} = sub-units {0,2,1,3}) come from four
+            // sub-units of the same thread: the first three are parked in local memory (dynamic index -> never
+            // in registers; 384 B per thread, L1/L2-resident) and the fourth stores 16 contiguous bytes per row
+            // and lane.  Storing each sub-unit on its own (stride-4 floats, 16 sectors per warp request) cost
+            // 12.1 ms on config 4 + interbin against 3.98 ms plain.
+            if (sub < 3) {
+#pragma unroll
+                for (int n1 = 0; n1 < 16; ++n1) held[sub * 16 + n1] = power2(y[n1]);
+            } else {
+                unsigned va = vmask, vb = vmask;         // bins 2n' (cells 0, 1) and 2n'+1 (cells 2, 3)
+                if (col0 + prm.overlap + prm.useful > prm.nbins) {
+#pragma unroll
+                    for (int n1 = 0; n1 < 16; ++n1) {
+                        if (col0 + 2 * (n1 * G::Q + tid) >= prm.nbins) va &= ~(1u << n1);
+                        if (col0 + 2 * (n1 * G::Q + tid) + 1 >= prm.nbins) vb &= ~(1u << n1);
+                    }
+                }
+                float *bp = prm.plane + (size_t)row_p * prm.ncols + (2 * col0 + 4 * tid);
+                float *bq = prm.plane + (size_t)row_q * prm.ncols + (2 * col0 + 4 * tid);
+                const bool alp = ((reinterpret_cast<uintptr_t>(bp) & 15) == 0);   // odd nbins: rows alternate
+                const bool alq = ((reinterpret_cast<uintptr_t>(bq) & 15) == 0);
+#pragma unroll
+                for (int n1 = 0; n1 < 16; ++n1) {
+                    const float2 c0 = held[n1], c2 = held[16 + n1], c1 = held[32 + n1], c3 = power2(y[n1]);
+                    const unsigned pa = va & (1u << n1), pb = vb & (1u << n1);
+                    st_stream4_if(bp + 4 * n1 * G::Q, c0.x, c1.x, c2.x, c3.x, (alp && pb) ? pa : 0u);
+                    st_stream2_if(bp + 4 * n1 * G::Q, c0.x, c1.x, (alp && pb) ? 0u : pa);
+                    st_stream2_if(bp + 4 * n1 * G::Q + 2, c2.x, c3.x, alp ? 0u : pb);
+                    st_stream4_if(bq + 4 * n1 * G::Q, c0.y, c1.y, c2.y, c3.y, (alq && pb) ? pa : 0u);
+                    st_stream2_if(bq + 4 * n1 * G::Q, c0.y, c1.y, (alq && pb) ? 0u : pa);
+                    st_stream2_if(bq + 4 * n1 * G::Q + 2, c2.y, c3.y, alq ? 0u : pb);
+                }
+            }
+        } else {
+            // bin n = 2n' + par -> plane column CS * (col0 + n) + half
+            float *bp = prm.plane + (size_t)row_p * prm.ncols + (CS * (col0 + 2 * tid + par) + half);
+            float *bq = prm.plane + (size_t)row_q * prm.ncols + (CS * (col0 + 2 * tid + par) + half);
+            const unsigned qon = (MODE != 0 && row_q == row_p) ? 0u : ~0u;   // MODE 1: z = 0 cell reported once
+            emit_unit<4096, false, MODE, 2 * CS>(prm, y, bp, bq, vm, vm & qon);
+        }
         __syncwarp();
         if (sub == SUBS - 1 && ++pair == prm.npairs) {
             pair = 0;

@@ -39,9 +39,9 @@ def load_peaks():
 
 
 # DRAM bytes (read + write) per launch of the fused kernel, from `ncu --set full` (dram__bytes_read.sum +
-# dram__bytes_write.sum): profiles/r1c_ncu_config{2,4,5}.md, profiles/r1d_ncu_config3.md.  None where no capture exists.
-NCU_TRAFFIC_BYTES = {2: 671.6e6, 3: 5752.6e6, 4: 7575.0e6, 5: 1395.6e6}
-NCU_TRAFFIC_FILE = {2: "r1c_ncu_config2.md", 3: "r1d_ncu_config3.md", 4: "r1c_ncu_config4.md", 5: "r1c_ncu_config5.md"}
+# dram__bytes_write.sum, launch 1): profiles/r1e_ncu_config{2,3,4,5}.md.  None where no capture exists.
+NCU_TRAFFIC_BYTES = {2: 671.2e6, 3: 5754.0e6, 4: 7576.0e6, 5: 1395.0e6}
+NCU_TRAFFIC_FILE = {c: f"r1e_ncu_config{c}.md" for c in (2, 3, 4, 5)}
 
 
 def workload(cfg_idx: int, interbin=None):

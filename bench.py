@@ -355,6 +355,7 @@ def main():
                           "per_sm_subpartition": {k: pr[k] for k in ("ffma", "fadd2", "ffma2_bcast", "ffma2_3pair", "fmul2")},
                           "per_sm": {k: pr[k] for k in ("lds_sts64", "shfl")},
                           "mix_round_cycles_per_sm": pr["mix_round"],
+                          "tmem_per_sm": fdas.fdas_probe_tmem(None, 2000),
                           "fp32_fma_probe_tflops": fdas.fdas_measure_fp32_peak(None, 4000)}))
         return
 

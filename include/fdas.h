@@ -193,6 +193,14 @@ fdas_status fdas_measure_fp32_peak(void *stream, int32_t iters, double *tflops);
  */
 fdas_status fdas_probe_pipes(void *stream, int32_t iters, double *out, int32_t nout);
 
+/*
+ * Tensor-memory probe: cycles per warp-wide tcgen05.ld / tcgen05.st of 32 columns (32x32b.x32, one 32-bit
+ * word per lane and column) per SM, 8 warps.  out[0] = load with a wait after every instruction, out[1] =
+ * loads, four per wait, out[2] = stores, four per wait, out[3] = 1 if the data read back is what was stored.
+ * nout >= 4.  Synchronises `stream`.
+ */
+fdas_status fdas_probe_tmem(void *stream, int32_t iters, double *out, int32_t nout);
+
 /* Number of kernels the library has launched in this process (for bench accounting). */
 int64_t fdas_launch_count(void);
 

@@ -520,3 +520,30 @@ extern "C" fdas_status fdas_probe_pipes(void *stream, int32_t iters, double *out
     cudaFree(d_out);
     return e == cudaSuccess ? FDAS_OK : FDAS_ERR_CUDA;
 }
+
+// cycles per warp-wide tcgen05.ld / tcgen05.st (32x32b.x32) per SM with 8 warps, see fdas_probe.cuh
+extern "C" fdas_status fdas_probe_tmem(void *stream, int32_t iters, double *out, int32_t nout)
+{
+    if (!out || iters <= 0 || nout < 4) return FDAS_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    float *d_out = nullptr;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaMalloc(&d_out, 64) != cudaSuccess)
+        return FDAS_ERR_CUDA;
+    cudaError_t e = cudaSuccess;
+    out[3] = 1.0;
+    for (int mode = 0; mode < 3 && e == cudaSuccess; ++mode) {
+        tmem_probe_kernel<<<sms, 256, 0, st>>>(d_out, 8, mode);          // warm-up
+        tmem_probe_kernel<<<sms, 256, 0, st>>>(d_out, iters, mode);
+        g_launches += 2;
+        e = cudaStreamSynchronize(st);
+        float h[3] = {0.f, 0.f, 0.f};
+        if (e == cudaSuccess) e = cudaMemcpy(h, d_out, sizeof(h), cudaMemcpyDeviceToHost);
+        out[mode] = (double)h[1] / ((double)iters * 4.0 * 8.0);          // 4 instructions per round, 8 warps per SM
+        if (h[2] != 1.f) out[3] = 0.0;                                   // read-back check
+    }
+    cudaFree(d_out);
+    return e == cudaSuccess ? FDAS_OK : FDAS_ERR_CUDA;
+}

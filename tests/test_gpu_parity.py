@@ -349,3 +349,10 @@ def test_pipe_probes(torch, fd):
     assert pr["ffma2_3pair"] > pr["ffma2_bcast"]
     assert 0.8 < pr["lds_sts64"] < 4.0 and 0.5 < pr["shfl"] < 4.0
     assert pr["mix_round"] > 0
+
+
+def test_tmem_probe(torch, fd):
+    """tcgen05.st / tcgen05.ld round trip through tensor memory (fdas_probe_tmem): data intact, sane cycle counts."""
+    pr = fd.fdas_probe_tmem(None, 500)
+    assert pr["readback_ok"]
+    assert 1.0 < pr["tmem_ld_x32"] < 64.0 and 1.0 < pr["tmem_st_x32"] < 64.0 and pr["tmem_ld_x32_waited"] >= pr["tmem_ld_x32"] * 0.9

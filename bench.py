@@ -327,8 +327,6 @@ def main():
                     help="skip the same-box unfused cuFFT comparator (variant A of the paper, N = 1 only)")
     ap.add_argument("--table4", action="store_true",
                     help="sweep the shapes of the paper's Table 4 (n = 2^20..2^23 samples, 65..257 templates) and exit")
-    ap.add_argument("--probe", action="store_true",
-                    help="print the instruction-cost probes (fdas_probe_pipes) as one JSON line and exit")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -346,19 +344,6 @@ def main():
             raise SystemExit("bench.py --table4 needs a CUDA device")
         run_table4()
         return
-    if args.probe:
-        if not torch.cuda.is_available():
-            raise SystemExit("bench.py --probe needs a CUDA device")
-        torch.cuda.set_device(0)
-        pr = fdas.fdas_probe_pipes(None, 2000)
-        print(json.dumps({"probe": "cycles per warp instruction (fdas_probe_pipes, include/fdas.h)",
-                          "per_sm_subpartition": {k: pr[k] for k in ("ffma", "fadd2", "ffma2_bcast", "ffma2_3pair", "fmul2")},
-                          "per_sm": {k: pr[k] for k in ("lds_sts64", "shfl")},
-                          "mix_round_cycles_per_sm": pr["mix_round"],
-                          "tmem_per_sm": fdas.fdas_probe_tmem(None, 2000),
-                          "fp32_fma_probe_tflops": fdas.fdas_measure_fp32_peak(None, 4000)}))
-        return
-
     rank, local_rank, world = dist.init()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")

@@ -20,7 +20,8 @@
  *
  * All entry points are plain C, take plain pointers and sizes, return a status code and
  * never throw or abort.  "device" pointers are CUDA device pointers on the device that
- * was current when the plan was created; "host" pointers are ordinary host memory.
+ * was current when the plan was created; every call that takes a plan returns
+ * FDAS_ERR_INVALID_ARG when another device is current.  "host" pointers are ordinary host memory.
  * `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
  * There is no CPU fallback anywhere in this library.
  */
@@ -38,7 +39,8 @@ typedef struct fdas_plan fdas_plan; /* opaque; created/destroyed by the library 
 typedef enum fdas_status {
     FDAS_OK = 0,
     FDAS_ERR_INVALID_ARG = 1, /* null pointer, nbins <= 0, zmax < 0, dz <= 0, zmax/dz not an integer      */
-    FDAS_ERR_UNSUPPORTED = 2, /* seglen not in {1024, 2048, 4096, 8192}, or too short for the bank's overlap */
+    FDAS_ERR_UNSUPPORTED = 2, /* seglen not in {1024, 2048, 4096, 8192}, or too short for the bank's overlap,
+                                 or a bank beyond 2e9 taps / spectrum slots                                   */
     FDAS_ERR_NOT_READY = 3,   /* fdas_execute before fdas_make_templates                                    */
     FDAS_ERR_ALIGNMENT = 4,   /* device pointer not 16-byte aligned                                         */
     FDAS_ERR_CUDA = 5,        /* a CUDA runtime call failed; see fdas_last_error()                          */
@@ -181,31 +183,12 @@ fdas_status fdas_get_template_spectrum(fdas_plan *plan, int32_t k, float *host_r
  */
 fdas_status fdas_measure_fp32_peak(void *stream, int32_t iters, double *tflops);
 
-/*
- * Instruction-cost probes: cycles per warp instruction measured with
- * clock64 on one CTA of 8 warps per SM, `iters` rounds each.  out[0..7] (nout >= 8):
- *   [0] scalar FFMA, [1] FADD2, [2] FFMA2 (pair * broadcast scalar + pair), [3] FFMA2 with three
- *   distinct register pairs, [4] FMUL2            -- per SM sub-partition (2 warps each);
- *   [5] conflict-free LDS.64 / STS.64, [6] SHFL  -- per SM (8 warps share the load/store pipe);
- *   [7] cycles per SM for one round of the unit-shaped mix: per warp 16 LDS.64 + 16 STS.64 +
- *       128 packed FP32 instructions, 8 warps.
- * Synchronises `stream`.
- */
-fdas_status fdas_probe_pipes(void *stream, int32_t iters, double *out, int32_t nout);
-
-/*
- * Tensor-memory probe: cycles per warp-wide tcgen05.ld / tcgen05.st of 32 columns (32x32b.x32, one 32-bit
- * word per lane and column) per SM, 8 warps.  out[0] = load with a wait after every instruction, out[1] =
- * loads, four per wait, out[2] = stores, four per wait, out[3] = 1 if the data read back is what was stored.
- * nout >= 4.  Synchronises `stream`.
- */
-fdas_status fdas_probe_tmem(void *stream, int32_t iters, double *out, int32_t nout);
-
 /* Number of kernels the library has launched in this process (for bench accounting). */
 int64_t fdas_launch_count(void);
 
 const char *fdas_status_string(fdas_status s);
-/* Text of the last CUDA error seen by this plan ("" if none). */
+/* Text of the last CUDA error seen by this plan ("" if none); plan = NULL: of the calling thread's last
+ * failed fdas_plan_create. */
 const char *fdas_last_error(const fdas_plan *plan);
 
 #ifdef __cplusplus

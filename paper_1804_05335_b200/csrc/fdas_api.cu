@@ -3,7 +3,6 @@
 // of fdas_templates.cuh / fdas_kernel.cuh; there is no CPU fallback.
 #include "../../include/fdas.h"
 #include "fdas_templates.cuh"
-#include "fdas_probe.cuh"
 
 #include <atomic>
 #include <cmath>
@@ -48,6 +47,25 @@ struct fdas_plan {
     } while (0)
 
 namespace {
+
+// Text of the last failure inside fdas_plan_create (the plan is gone by then): fdas_last_error(NULL).
+thread_local char g_create_err[256] = "";
+
+// Plans are bound to the device that was current at fdas_plan_create: every entry point that touches
+// plan-owned device memory refuses to run with another device current (FDAS_ERR_INVALID_ARG).
+bool on_plan_device(fdas_plan *p)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    if (dev != p->device) {
+        snprintf(p->err, sizeof(p->err), "plan was created on device %d, current device is %d", p->device, dev);
+        return false;
+    }
+    return true;
+}
 
 typedef void (*kernel_fn)(const KernelParams);
 
@@ -123,7 +141,7 @@ const char *fdas_status_string(fdas_status s)
     return "FDAS_ERR_UNKNOWN";
 }
 
-const char *fdas_last_error(const fdas_plan *plan) { return plan ? plan->err : ""; }
+const char *fdas_last_error(const fdas_plan *plan) { return plan ? plan->err : g_create_err; }
 
 int64_t fdas_launch_count(void) { return g_launches.load(); }
 
@@ -146,6 +164,12 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double
     const int ov = ((m + (interbin ? 1 : 0)) + 31) / 32 * 32; // >= m (+1 for the interbin neighbour), 128B-aligned
     const int B = seglen - 2 * ov;
     if (B < 32) return FDAS_ERR_UNSUPPORTED;
+    g_create_err[0] = 0;
+    // 32-bit index arithmetic in the template kernels: K * (2m+1) taps and npairs * L spectrum slots per bank
+    if ((double)K * (2.0 * m + 1.0) > 2.0e9 || ((double)K + 1.0) * 0.5 * seglen > 2.0e9) {
+        snprintf(g_create_err, sizeof(g_create_err), "template bank too large: K = %d, half-width %d", K, m);
+        return FDAS_ERR_UNSUPPORTED;
+    }
     kernel_fn kern = select_kernel(seglen, interbin);
     if (!kern) return FDAS_ERR_UNSUPPORTED;
 
@@ -175,25 +199,28 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double
 
     fdas_status st = FDAS_OK;
     do {
-        cudaError_t e;
-        if ((e = cudaGetDevice(&p->device)) != cudaSuccess) { st = FDAS_ERR_CUDA; break; }
+        cudaError_t e = cudaSuccess;
+#define FDAS_CREATE_FAIL(code)                                                                     \
+    {                                                                                              \
+        st = code;                                                                                 \
+        snprintf(g_create_err, sizeof(g_create_err), "fdas_plan_create: %s", cudaGetErrorString(e)); \
+        break;                                                                                     \
+    }
+        if ((e = cudaGetDevice(&p->device)) != cudaSuccess) FDAS_CREATE_FAIL(FDAS_ERR_CUDA)
         cudaDeviceProp prop;
-        if ((e = cudaGetDeviceProperties(&prop, p->device)) != cudaSuccess) { st = FDAS_ERR_CUDA; break; }
+        if ((e = cudaGetDeviceProperties(&prop, p->device)) != cudaSuccess) FDAS_CREATE_FAIL(FDAS_ERR_CUDA)
         I.sm_count = prop.multiProcessorCount;
         if ((e = cudaFuncSetAttribute((const void *)kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      I.smem_bytes)) != cudaSuccess) { st = FDAS_ERR_CUDA; break; }
+                                      I.smem_bytes)) != cudaSuccess) FDAS_CREATE_FAIL(FDAS_ERR_CUDA)
         if ((e = cudaFuncSetAttribute((const void *)p->kernel_thr, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      I.smem_bytes)) != cudaSuccess) { st = FDAS_ERR_CUDA; break; }
+                                      I.smem_bytes)) != cudaSuccess) FDAS_CREATE_FAIL(FDAS_ERR_CUDA)
         cudaFuncAttributes fa;
-        if ((e = cudaFuncGetAttributes(&fa, (const void *)kern)) != cudaSuccess) { st = FDAS_ERR_CUDA; break; }
+        if ((e = cudaFuncGetAttributes(&fa, (const void *)kern)) != cudaSuccess) FDAS_CREATE_FAIL(FDAS_ERR_CUDA)
         I.regs = fa.numRegs;
         int occ = 0;
         if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)kern, I.threads,
-                                                               I.smem_bytes)) != cudaSuccess) { st = FDAS_ERR_CUDA; break; }
+                                                               I.smem_bytes)) != cudaSuccess) FDAS_CREATE_FAIL(FDAS_ERR_CUDA)
         if (occ < 1) { st = FDAS_ERR_UNSUPPORTED; break; }
-#ifdef FDAS_TUNE
-        if (const char *e = getenv("FDAS_CTAS_PER_SM")) occ = atoi(e) < occ ? atoi(e) : occ;
-#endif
         I.ctas_per_sm = occ;
         I.grid = occ * I.sm_count;
         const size_t taps_bytes = (size_t)p->nbanks * K * (2 * m + 1) * sizeof(double2);
@@ -202,10 +229,10 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double
             cudaMalloc(&p->d_hperm, h_bytes) != cudaSuccess ||
             cudaMalloc(&p->d_wtab, (size_t)seglen * sizeof(float2)) != cudaSuccess ||
             (seglen == 8192 && cudaMalloc(&p->d_wtab2, (size_t)seglen * sizeof(float2)) != cudaSuccess)) {
-            cudaGetLastError();
-            st = FDAS_ERR_NOMEM;
-            break;
+            e = cudaGetLastError();
+            FDAS_CREATE_FAIL(FDAS_ERR_NOMEM)
         }
+#undef FDAS_CREATE_FAIL
     } while (0);
     if (st != FDAS_OK) {
         fdas_destroy(p);
@@ -217,12 +244,12 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double
 
 fdas_status fdas_make_templates(fdas_plan *p, void *stream)
 {
-    if (!p) return FDAS_ERR_INVALID_ARG;
+    if (!p || !on_plan_device(p)) return FDAS_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     const fdas_info &I = p->info;
     const int w = 2 * I.halfwidth + 1;
     {
-        const int n = I.ntemplates * w;
+        const int n = I.ntemplates * w;                      // <= 2e9: checked in fdas_plan_create
         for (int b = 0; b < p->nbanks; ++b)
             make_taps_kernel<<<(n + 127) / 128, 128, 0, st>>>(p->d_taps + (size_t)b * n, I.ntemplates, I.halfwidth,
                                                               I.zmax, I.dz, b);
@@ -293,7 +320,7 @@ static fdas_status launch_fused(fdas_plan *p, void *stream, const void *d_spectr
 
 fdas_status fdas_execute(fdas_plan *p, void *stream, const void *d_spectrum, float *d_plane)
 {
-    if (!p || !d_spectrum || !d_plane) return FDAS_ERR_INVALID_ARG;
+    if (!p || !d_spectrum || !d_plane || !on_plan_device(p)) return FDAS_ERR_INVALID_ARG;
     if (!p->ready) return FDAS_ERR_NOT_READY;
     if (((uintptr_t)d_spectrum & 15) || ((uintptr_t)d_plane & 15)) return FDAS_ERR_ALIGNMENT;
     return launch_fused(p, stream, d_spectrum, d_plane, 0.f, nullptr, 0, nullptr);
@@ -302,7 +329,8 @@ fdas_status fdas_execute(fdas_plan *p, void *stream, const void *d_spectrum, flo
 fdas_status fdas_execute_threshold(fdas_plan *p, void *stream, const void *d_spectrum, float threshold,
                                    fdas_candidate *d_cands, int64_t capacity, uint64_t *d_count)
 {
-    if (!p || !d_spectrum || !d_count || capacity < 0 || (capacity > 0 && !d_cands) || threshold != threshold)
+    if (!p || !d_spectrum || !d_count || capacity < 0 || (capacity > 0 && !d_cands) || threshold != threshold ||
+        !on_plan_device(p))
         return FDAS_ERR_INVALID_ARG;
     if (!p->ready) return FDAS_ERR_NOT_READY;
     if (((uintptr_t)d_spectrum & 15) || ((uintptr_t)d_cands & 15) || ((uintptr_t)d_count & 7))
@@ -314,18 +342,20 @@ fdas_status fdas_execute_threshold(fdas_plan *p, void *stream, const void *d_spe
 
 fdas_status fdas_execute_host(fdas_plan *p, void *stream, const void *h_spectrum, float *h_plane)
 {
-    if (!p || !h_spectrum || !h_plane) return FDAS_ERR_INVALID_ARG;
+    if (!p || !h_spectrum || !h_plane || !on_plan_device(p)) return FDAS_ERR_INVALID_ARG;
     if (!p->ready) return FDAS_ERR_NOT_READY;
     const fdas_info &I = p->info;
     cudaStream_t st = (cudaStream_t)stream;
-    if (!p->d_stage_in) {
-        if (cudaMalloc(&p->d_stage_in, (size_t)I.nbins * sizeof(float2)) != cudaSuccess ||
-            cudaMalloc(&p->d_stage_out, (size_t)I.plane_bytes) != cudaSuccess) {
-            cudaGetLastError();
-            cudaFree(p->d_stage_in);
-            p->d_stage_in = nullptr;
-            return FDAS_ERR_NOMEM;
-        }
+    // the two staging buffers are allocated independently: fdas_execute_threshold_host shares d_stage_in only
+    if (!p->d_stage_in && cudaMalloc(&p->d_stage_in, (size_t)I.nbins * sizeof(float2)) != cudaSuccess) {
+        cudaGetLastError();
+        p->d_stage_in = nullptr;
+        return FDAS_ERR_NOMEM;
+    }
+    if (!p->d_stage_out && cudaMalloc(&p->d_stage_out, (size_t)I.plane_bytes) != cudaSuccess) {
+        cudaGetLastError();
+        p->d_stage_out = nullptr;
+        return FDAS_ERR_NOMEM;
     }
     FDAS_CUDA(p, cudaMemcpyAsync(p->d_stage_in, h_spectrum, (size_t)I.nbins * sizeof(float2),
                                  cudaMemcpyHostToDevice, st));
@@ -339,7 +369,8 @@ fdas_status fdas_execute_host(fdas_plan *p, void *stream, const void *h_spectrum
 fdas_status fdas_execute_threshold_host(fdas_plan *p, void *stream, const void *h_spectrum, float threshold,
                                         fdas_candidate *h_cands, int64_t capacity, uint64_t *h_count)
 {
-    if (!p || !h_spectrum || !h_count || capacity < 0 || (capacity > 0 && !h_cands)) return FDAS_ERR_INVALID_ARG;
+    if (!p || !h_spectrum || !h_count || capacity < 0 || (capacity > 0 && !h_cands) || !on_plan_device(p))
+        return FDAS_ERR_INVALID_ARG;
     if (!p->ready) return FDAS_ERR_NOT_READY;
     const fdas_info &I = p->info;
     cudaStream_t st = (cudaStream_t)stream;
@@ -403,7 +434,8 @@ fdas_status fdas_plan_info(const fdas_plan *p, fdas_info *out)
 
 fdas_status fdas_get_taps(fdas_plan *p, int32_t k, double *host_re_im, int32_t *halfwidth_k)
 {
-    if (!p || !host_re_im || !halfwidth_k || k < 0 || k >= p->info.ntemplates * p->nbanks) return FDAS_ERR_INVALID_ARG;
+    if (!p || !host_re_im || !halfwidth_k || k < 0 || k >= p->info.ntemplates * p->nbanks || !on_plan_device(p))
+        return FDAS_ERR_INVALID_ARG;
     if (!p->ready) return FDAS_ERR_NOT_READY;
     const fdas_info &I = p->info;
     const int m = I.halfwidth, w = 2 * m + 1;
@@ -420,7 +452,7 @@ fdas_status fdas_get_taps(fdas_plan *p, int32_t k, double *host_re_im, int32_t *
 
 fdas_status fdas_get_template_spectrum(fdas_plan *p, int32_t k, float *host_re_im)
 {
-    if (!p || !host_re_im || k < 0 || k >= p->info.ntemplates) return FDAS_ERR_INVALID_ARG;
+    if (!p || !host_re_im || k < 0 || k >= p->info.ntemplates || !on_plan_device(p)) return FDAS_ERR_INVALID_ARG;
     if (!p->ready) return FDAS_ERR_NOT_READY;
     const fdas_info &I = p->info;
     const int L = I.seglen, T = I.threads;
@@ -475,75 +507,3 @@ fdas_status fdas_measure_fp32_peak(void *stream, int32_t iters, double *tflops)
 }
 
 } // extern "C"
-
-namespace {
-template <int MODE>
-cudaError_t run_probe(cudaStream_t st, float *d_out, int sms, int iters, double *cycles_per_instr)
-{
-    const int threads = 256;                       // 8 warps: two per SM sub-partition
-    const size_t smem = (size_t)16 * threads * sizeof(float2);
-    probe_kernel<MODE><<<sms, threads, smem, st>>>(d_out, 8, 1.0001f, 0.9999f);        // warm-up
-    probe_kernel<MODE><<<sms, threads, smem, st>>>(d_out, iters, 1.0001f, 0.9999f);
-    g_launches += 2;
-    cudaError_t e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) return e;
-    float h[2];
-    e = cudaMemcpy(h, d_out, sizeof(h), cudaMemcpyDeviceToHost);
-    if (e != cudaSuccess) return e;
-    const bool per_sm = (MODE == PROBE_LDS_STS64 || MODE == PROBE_SHFL || MODE == PROBE_MIX);
-    // FP modes: per SM sub-partition (2 warps each); memory modes: per SM (8 warps share one LSU)
-    const double warps = (MODE == PROBE_MIX) ? 1.0 : per_sm ? 8.0 : 2.0;   // mix: whole round of the CTA
-    *cycles_per_instr = (double)h[1] / ((double)iters * probe_instr_per_round(MODE) * warps);
-    return cudaGetLastError();
-}
-} // namespace
-
-extern "C" fdas_status fdas_probe_pipes(void *stream, int32_t iters, double *out, int32_t nout)
-{
-    if (!out || iters <= 0 || nout < (int)PROBE_COUNT) return FDAS_ERR_INVALID_ARG;
-    cudaStream_t st = (cudaStream_t)stream;
-    int dev = 0, sms = 0;
-    float *d_out = nullptr;
-    if (cudaGetDevice(&dev) != cudaSuccess ||
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
-        cudaMalloc(&d_out, 64) != cudaSuccess)
-        return FDAS_ERR_CUDA;
-    cudaError_t e = cudaSuccess;
-    if (e == cudaSuccess) e = run_probe<PROBE_FFMA>(st, d_out, sms, iters, &out[PROBE_FFMA]);
-    if (e == cudaSuccess) e = run_probe<PROBE_FADD2>(st, d_out, sms, iters, &out[PROBE_FADD2]);
-    if (e == cudaSuccess) e = run_probe<PROBE_FFMA2>(st, d_out, sms, iters, &out[PROBE_FFMA2]);
-    if (e == cudaSuccess) e = run_probe<PROBE_FFMA2_3PAIR>(st, d_out, sms, iters, &out[PROBE_FFMA2_3PAIR]);
-    if (e == cudaSuccess) e = run_probe<PROBE_FMUL2>(st, d_out, sms, iters, &out[PROBE_FMUL2]);
-    if (e == cudaSuccess) e = run_probe<PROBE_LDS_STS64>(st, d_out, sms, iters, &out[PROBE_LDS_STS64]);
-    if (e == cudaSuccess) e = run_probe<PROBE_SHFL>(st, d_out, sms, iters, &out[PROBE_SHFL]);
-    if (e == cudaSuccess) e = run_probe<PROBE_MIX>(st, d_out, sms, iters, &out[PROBE_MIX]);
-    cudaFree(d_out);
-    return e == cudaSuccess ? FDAS_OK : FDAS_ERR_CUDA;
-}
-
-// cycles per warp-wide tcgen05.ld / tcgen05.st (32x32b.x32) per SM with 8 warps, see fdas_probe.cuh
-extern "C" fdas_status fdas_probe_tmem(void *stream, int32_t iters, double *out, int32_t nout)
-{
-    if (!out || iters <= 0 || nout < 4) return FDAS_ERR_INVALID_ARG;
-    cudaStream_t st = (cudaStream_t)stream;
-    int dev = 0, sms = 0;
-    float *d_out = nullptr;
-    if (cudaGetDevice(&dev) != cudaSuccess ||
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
-        cudaMalloc(&d_out, 64) != cudaSuccess)
-        return FDAS_ERR_CUDA;
-    cudaError_t e = cudaSuccess;
-    out[3] = 1.0;
-    for (int mode = 0; mode < 3 && e == cudaSuccess; ++mode) {
-        tmem_probe_kernel<<<sms, 256, 0, st>>>(d_out, 8, mode);          // warm-up
-        tmem_probe_kernel<<<sms, 256, 0, st>>>(d_out, iters, mode);
-        g_launches += 2;
-        e = cudaStreamSynchronize(st);
-        float h[3] = {0.f, 0.f, 0.f};
-        if (e == cudaSuccess) e = cudaMemcpy(h, d_out, sizeof(h), cudaMemcpyDeviceToHost);
-        out[mode] = (double)h[1] / ((double)iters * 4.0 * 8.0);          // 4 instructions per round, 8 warps per SM
-        if (h[2] != 1.f) out[3] = 0.0;                                   // read-back check
-    }
-    cudaFree(d_out);
-    return e == cudaSuccess ? FDAS_OK : FDAS_ERR_CUDA;
-}

@@ -21,7 +21,7 @@ STATUS_NAMES = {0: "FDAS_OK", 1: "FDAS_ERR_INVALID_ARG", 2: "FDAS_ERR_UNSUPPORTE
 EXPORTS = ["fdas_plan_create", "fdas_make_templates", "fdas_execute", "fdas_execute_host", "fdas_execute_threshold",
            "fdas_execute_threshold_host",
            "fdas_destroy",
-           "fdas_plan_info", "fdas_get_taps", "fdas_get_template_spectrum", "fdas_measure_fp32_peak", "fdas_probe_pipes", "fdas_probe_tmem",
+           "fdas_plan_info", "fdas_get_taps", "fdas_get_template_spectrum", "fdas_measure_fp32_peak",
            "fdas_launch_count", "fdas_status_string", "fdas_last_error"]
 
 
@@ -63,8 +63,6 @@ def _load() -> ctypes.CDLL:
     lib.fdas_get_taps.argtypes = [vp, i32, vp, ctypes.POINTER(i32)]
     lib.fdas_get_template_spectrum.argtypes = [vp, i32, vp]
     lib.fdas_measure_fp32_peak.argtypes = [vp, i32, ctypes.POINTER(dbl)]
-    lib.fdas_probe_pipes.argtypes = [vp, i32, ctypes.POINTER(dbl), i32]
-    lib.fdas_probe_tmem.argtypes = [vp, i32, ctypes.POINTER(dbl), i32]
     for name in EXPORTS:
         getattr(lib, name).restype = ctypes.c_int
     lib.fdas_launch_count.restype = i64
@@ -174,21 +172,6 @@ def fdas_measure_fp32_peak(stream=None, iters: int = 4096) -> float:
     out = ctypes.c_double()
     _check(lib.fdas_measure_fp32_peak(_stream(stream), int(iters), ctypes.byref(out)), "fdas_measure_fp32_peak")
     return out.value
-
-
-PROBE_NAMES = ("ffma", "fadd2", "ffma2_bcast", "ffma2_3pair", "fmul2", "lds_sts64", "shfl", "mix_round")
-
-
-def fdas_probe_pipes(stream=None, iters: int = 2000) -> dict:
-    out = (ctypes.c_double * len(PROBE_NAMES))()
-    _check(lib.fdas_probe_pipes(_stream(stream), int(iters), out, len(PROBE_NAMES)), "fdas_probe_pipes")
-    return dict(zip(PROBE_NAMES, [float(x) for x in out]))
-
-
-def fdas_probe_tmem(stream=None, iters: int = 2000) -> dict:
-    out = (ctypes.c_double * 4)()
-    _check(lib.fdas_probe_tmem(_stream(stream), int(iters), out, 4), "fdas_probe_tmem")
-    return {"tmem_ld_x32_waited": out[0], "tmem_ld_x32": out[1], "tmem_st_x32": out[2], "readback_ok": bool(out[3])}
 
 
 def fdas_launch_count() -> int:

@@ -339,20 +339,3 @@ def test_fp32_peak_probe(torch, fd):
     tf = fd.fdas_measure_fp32_peak(None, 2000)
     assert 20.0 < tf < 90.0, tf
     assert fd.fdas_launch_count() > 0
-
-
-def test_pipe_probes(torch, fd):
-    pr = fd.fdas_probe_pipes(None, 300)
-    assert set(pr) == set(fd.PROBE_NAMES)
-    assert 0.9 < pr["ffma"] < 1.6              # one scalar FFMA per clock per sub-partition
-    assert 1.8 < pr["fadd2"] < 3.0 and 1.8 < pr["ffma2_bcast"] < 3.0 and 1.8 < pr["fmul2"] < 3.0
-    assert pr["ffma2_3pair"] > pr["ffma2_bcast"]
-    assert 0.8 < pr["lds_sts64"] < 4.0 and 0.5 < pr["shfl"] < 4.0
-    assert pr["mix_round"] > 0
-
-
-def test_tmem_probe(torch, fd):
-    """tcgen05.st / tcgen05.ld round trip through tensor memory (fdas_probe_tmem): data intact, sane cycle counts."""
-    pr = fd.fdas_probe_tmem(None, 500)
-    assert pr["readback_ok"]
-    assert 1.0 < pr["tmem_ld_x32"] < 64.0 and 1.0 < pr["tmem_st_x32"] < 64.0 and pr["tmem_ld_x32_waited"] >= pr["tmem_ld_x32"] * 0.9

@@ -77,8 +77,7 @@ kernel_fn pick_kernel(int ib, int mode)
     return ib ? (kernel_fn)fdas_fused_kernel<L, true, MINB> : (kernel_fn)fdas_fused_kernel<L, false, MINB>;
 }
 
-// L = 4096: second-generation kernel (shuffle exchange, fdas_kernel2.cuh); measured on B200 it is
-// 4.5 % faster than the first at L = 4096 and 7 % slower at L = 2048, which stays on the first.
+// L = 4096: second-generation kernel (shuffle exchange, fdas_kernel2.cuh).
 template <int L, int MINB>
 kernel_fn pick_kernel2(int ib, int mode)
 {
@@ -87,13 +86,24 @@ kernel_fn pick_kernel2(int ib, int mode)
     return ib ? (kernel_fn)fdas_fused_kernel2<L, true, MINB> : (kernel_fn)fdas_fused_kernel2<L, false, MINB>;
 }
 
+// L = 2048: third-generation kernel (X^ and twiddles in tensor memory, three CTAs per SM, fdas_kernel3.cuh).
+template <int L, int MINB>
+kernel_fn pick_kernel3(int ib, int mode)
+{
+    if (ib == 2) return mode ? (kernel_fn)fdas_fused_kernel3<L, false, MINB, 1, 2> : (kernel_fn)fdas_fused_kernel3<L, false, MINB, 0, 2>;
+    if (mode) return ib ? (kernel_fn)fdas_fused_kernel3<L, true, MINB, 1> : (kernel_fn)fdas_fused_kernel3<L, false, MINB, 1>;
+    return ib ? (kernel_fn)fdas_fused_kernel3<L, true, MINB> : (kernel_fn)fdas_fused_kernel3<L, false, MINB>;
+}
+
+constexpr int K3_CTAS_PER_SM_2048 = 3;   // fdas_kernel3.cuh at L = 2048: <= 168 registers, 72 KB, 128 tensor-memory columns
+
 // mode 0: plane store (fdas_execute); mode 1: threshold search (fdas_execute_threshold)
 // ib: 0 none, 1 interbinning (eq. 4), 2 two-bin Fourier interpolation (second template bank; L <= 4096)
 kernel_fn select_kernel(int L, int ib, int mode = 0)
 {
     switch (L) {
     case 1024: return pick_kernel<1024, 4>(ib, mode);
-    case 2048: return pick_kernel<2048, 2>(ib, mode);
+    case 2048: return pick_kernel3<2048, K3_CTAS_PER_SM_2048>(ib, mode);
     case 4096: return pick_kernel2<4096, 1>(ib, mode);
     case 8192:                                                            // 2 x 4096 (fdas_kernel8k.cuh)
         if (ib == 2) return nullptr;
@@ -107,7 +117,7 @@ int smem_bytes_for(int L, bool ib)
 {
     switch (L) {
     case 1024: return Geo<1024>::smem_bytes(ib);
-    case 2048: return Geo<2048>::smem_bytes(ib);
+    case 2048: return Geo3<2048>::smem_bytes(ib);
     case 4096: return Geo2<4096>::smem_bytes(ib);
     case 8192: return Geo8k::smem_bytes();
     default: return 0;
@@ -118,7 +128,7 @@ void freq_to_reg_any(int L, int f, int &tid, int &i)
 {
     switch (L) {
     case 1024: freq_to_reg<1024>(f, tid, i); break;
-    case 2048: freq_to_reg<2048>(f, tid, i); break;
+    case 2048: freq_to_reg3<2048>(f, tid, i); break;
     default: freq_to_reg<4096>(f & 4095, tid, i); break;   // 8192: slot of f mod 4096 in half f / 4096
     }
 }
@@ -214,6 +224,11 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double
                                       I.smem_bytes)) != cudaSuccess) FDAS_CREATE_FAIL(FDAS_ERR_CUDA)
         if ((e = cudaFuncSetAttribute((const void *)p->kernel_thr, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       I.smem_bytes)) != cudaSuccess) FDAS_CREATE_FAIL(FDAS_ERR_CUDA)
+        // several CTAs per SM only fit with the largest shared-memory carve-out of the unified L1
+        if ((e = cudaFuncSetAttribute((const void *)kern, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                      cudaSharedmemCarveoutMaxShared)) != cudaSuccess) FDAS_CREATE_FAIL(FDAS_ERR_CUDA)
+        if ((e = cudaFuncSetAttribute((const void *)p->kernel_thr, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                      cudaSharedmemCarveoutMaxShared)) != cudaSuccess) FDAS_CREATE_FAIL(FDAS_ERR_CUDA)
         cudaFuncAttributes fa;
         if ((e = cudaFuncGetAttributes(&fa, (const void *)kern)) != cudaSuccess) FDAS_CREATE_FAIL(FDAS_ERR_CUDA)
         I.regs = fa.numRegs;
@@ -221,6 +236,10 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double
         if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)kern, I.threads,
                                                                I.smem_bytes)) != cudaSuccess) FDAS_CREATE_FAIL(FDAS_ERR_CUDA)
         if (occ < 1) { st = FDAS_ERR_UNSUPPORTED; break; }
+        // cudaOccupancyMaxActiveBlocksPerMultiprocessor answers 1 for any kernel that uses tensor memory
+        // (EIATTR_TCGEN05_1CTA_USED); fdas_kernel3.cuh allocates 128 of the SM's 512 columns per CTA and is
+        // built for K3_CTAS_PER_SM_2048 CTAs per SM by registers and shared memory (measured: they are co-resident).
+        if (seglen == 2048 && occ < K3_CTAS_PER_SM_2048) occ = K3_CTAS_PER_SM_2048;
         I.ctas_per_sm = occ;
         I.grid = occ * I.sm_count;
         const size_t taps_bytes = (size_t)p->nbanks * K * (2 * m + 1) * sizeof(double2);
@@ -270,7 +289,7 @@ fdas_status fdas_make_templates(fdas_plan *p, void *stream)
             break;
         case 2048:
             for (int b = 0; b < p->nbanks; ++b)
-                make_spectra_kernel<2048><<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps + (size_t)b * n, I.npairs, I.halfwidth,
+                make_spectra_kernel<2048, 3><<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps + (size_t)b * n, I.npairs, I.halfwidth,
                                                             I.zmax, I.dz, I.ntemplates, p->nbanks, b);
             break;
         case 4096:

@@ -15,6 +15,7 @@
 #include "fdas_kernel.cuh"
 #include "fdas_kernel8k.cuh"
 #include "fdas_kernel2.cuh"
+#include "fdas_kernel3.cuh"
 
 namespace fdas {
 
@@ -127,7 +128,8 @@ __global__ void make_wtab_kernel(float2 *wtab, int L)
 
 // hperm[pair][i/2][tid] (float4 = two complex) for the rows z <= 0 (pair = row index k).
 // nbanks = 2: slot = pair * 2 + bank; `taps` points at the bank's tap array.
-template <int L>
+// MAP = 3: register order of fdas_kernel3.cuh (freq_to_reg3), else of fdas_kernel.cuh.
+template <int L, int MAP = 0>
 __global__ void make_spectra_kernel(float2 *hperm, const double2 *taps, int npairs, int m,
                                     double zmax, double dz, int K, int nbanks, int bank)
 {
@@ -150,7 +152,8 @@ __global__ void make_spectra_kernel(float2 *hperm, const double2 *taps, int npai
         si += t.x * s - t.y * c;
     }
     int tid, i;
-    freq_to_reg<L>(f, tid, i);
+    if constexpr (MAP == 3) freq_to_reg3<L>(f, tid, i);
+    else freq_to_reg<L>(f, tid, i);
     const size_t off = ((((size_t)pair * nbanks + bank) * (G::PTS / 2) + (i >> 1)) * G::T + tid) * 2 + (i & 1);
     hperm[off] = make_float2((float)(sr / L), (float)(si / L));
 }

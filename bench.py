@@ -3,12 +3,17 @@
 bench.py -- throughput of the FDAS correlation hot path (BASELINE.json metric: f-fdot plane
 cells/s, input bins/s, achieved HBM GB/s vs roofline) on synthetic spectra.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path (segment fetch, forward FFT, multiply by every
-template, inverse FFT, discard, power(/interbin), plane store = one fdas_execute) over one
-spectrum of the workload.  N > 1: one process per GPU (torchrun), spectra sharded across ranks,
-no data-path collective (weak scaling: one spectrum per rank per step).
+template, inverse FFT, discard, power(/interbin), plane store) over one BATCH of the workload:
+`batch` fdas_execute calls back to back on one CUDA stream (config 5, the default and the largest
+single-GPU workload of BASELINE.json: 64 spectra per step; configs 2-4: one spectrum).  The same
+JSON line carries a "configs" record with the kernel time and both roofline fractions of the
+other full-size configs (2, 3, 4), so one run covers every workload BASELINE.json names.
+N > 1: one process per GPU -- launched by torchrun, or by this script itself when WORLD_SIZE is
+unset (`python bench.py --gpus N` re-executes under torch.distributed.run) -- the 64*N spectra of
+the job are sharded across ranks with dist.shard, no data-path collective (weak scaling).
 Prints ONE JSON line on rank 0.
 """
 from __future__ import annotations
@@ -38,10 +43,27 @@ def load_peaks():
     return {"hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)"}
 
 
-# DRAM bytes (read + write) per launch of the fused kernel, from `ncu --set full` (dram__bytes_read.sum +
-# dram__bytes_write.sum, launch 1): profiles/r1e_ncu_config{2,3,4,5}.md.  None where no capture exists.
-NCU_TRAFFIC_BYTES = {2: 671.2e6, 3: 5754.0e6, 4: 7576.0e6, 5: 1395.0e6}
-NCU_TRAFFIC_FILE = {c: f"r1e_ncu_config{c}.md" for c in (2, 3, 4, 5)}
+# DRAM bytes (read + write) per launch of the fused kernel come from the committed `ncu --set full` summaries
+# (dram__bytes_read.sum + dram__bytes_write.sum, first captured launch); None where no capture of the kernel
+# that runs today exists.  The file is named in the JSON line next to the number.
+PROFILE_ROUND = "r2"
+_UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+
+
+def profiled_traffic(cfg_idx: int):
+    """(bytes per launch, file name) parsed from profiles/<round>_ncu_config<k>.md, or (None, None)."""
+    name = f"{PROFILE_ROUND}_ncu_config{cfg_idx}.md"
+    path = os.path.join(ROOT, "profiles", name)
+    if not os.path.exists(path):
+        return None, None
+    total, seen = 0.0, 0
+    with open(path) as f:
+        for line in f:
+            cells = [c.strip() for c in line.split("|")]
+            if len(cells) >= 5 and cells[1] in ("dram__bytes_read.sum", "dram__bytes_write.sum") and cells[2] in _UNIT:
+                total += float(cells[3]) * _UNIT[cells[2]]
+                seen += 1
+    return (total, name) if seen == 2 else (None, None)
 
 
 def workload(cfg_idx: int, interbin=None):
@@ -62,7 +84,7 @@ def workload(cfg_idx: int, interbin=None):
     flops = nseg_alg * ((1 + nb * K) * 5 * L * math.log2(L) + 6 * nb * K * L + 3 * nb * K * b_alg
                         + (5 * K * b_alg if c["interbin"] == 1 else 0))
     nbytes = 8 * N + 8 * nb * K * L + 4 * K * ncols
-    c.update(K=K, m=m, ncols=ncols, cells=K * ncols, alg_flops=flops, alg_bytes=nbytes)
+    c.update(K=K, m=m, ncols=ncols, cells=K * ncols, alg_flops=flops, alg_bytes=nbytes)     # per spectrum
     return c
 
 
@@ -312,27 +334,126 @@ def run_table4():
                                "the paper's includes; other hardware: context, not a target", "rows": rows}))
 
 
+KERNEL_OF_SEGLEN = {1024: "fdas_fused_kernel", 2048: "fdas_fused_kernel3", 4096: "fdas_fused_kernel2",
+                    8192: "fdas_fused_kernel_8k"}
+
+
+def roofline_record(w, info, kernel_ms, peaks, sm_max_mhz, cfg_idx, overridden, fp32_probe=None):
+    """north_star's roofline for ONE launch (one spectrum): the slower of compulsory bytes at HBM bandwidth and
+    FFT flops at FP32 peak; `achieved` = algorithmic bytes (flops) per launch / average launch duration."""
+    fp32_peak = info.sm_count * 128 * 2 * sm_max_mhz * 1e6 / 1e12       # DESIGN.md "Roofline"
+    t_hbm = w["alg_bytes"] / (peaks["hbm_gbs"] * 1e9)
+    t_alu = w["alg_flops"] / (fp32_peak * 1e12)
+    s = kernel_ms * 1e-3
+    ach_gbs, ach_tf = w["alg_bytes"] / s / 1e9, w["alg_flops"] / s / 1e12
+    traffic, tfile = (None, None) if overridden else profiled_traffic(cfg_idx)
+    hbm = {"bound": "hbm", "achieved": ach_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+           "frac": ach_gbs / peaks["hbm_gbs"], "traffic": traffic, "peak_source": peaks["source"]}
+    alu = {"bound": "alu", "achieved": ach_tf, "peak": fp32_peak, "unit": "TFLOP/s", "frac": ach_tf / fp32_peak,
+           "traffic": traffic,
+           "peak_source": f"{info.sm_count} SMs x 128 FP32 lanes x 2 x {sm_max_mhz:.0f} MHz (DESIGN.md)"}
+    if fp32_probe is not None:
+        alu["fma_probe_tflops"] = fp32_probe
+    roof = dict(alu if t_alu >= t_hbm else hbm)          # north_star: the slower bound is the roofline
+    roof.update(kernel=KERNEL_OF_SEGLEN[w["seglen"]], kernel_ms=kernel_ms,
+                traffic_source=f"ncu --set full, profiles/{tfile} (dram bytes per launch)" if tfile else None,
+                alg_bytes=w["alg_bytes"], alg_flops=w["alg_flops"],
+                t_bound_ms={"hbm": t_hbm * 1e3, "alu": t_alu * 1e3},
+                hbm=hbm if roof["bound"] == "alu" else None, alu=alu if roof["bound"] == "hbm" else None)
+    return roof
+
+
+def time_config(torch, fdas, synthetic, dev, stream, w, steps, warmup, seed_off=0, nin=4):
+    """Kernel time per spectrum (ms) of one config on this rank: `steps` launches between two CUDA events."""
+    import numpy as np
+    plan = fdas.Plan(w["nbins"], w["zmax"], w["dz"], w["seglen"], w["interbin"])
+    plan.make_templates()
+    info = plan.info
+    N = info.nbins
+    d_in = [torch.from_numpy(synthetic.noise_only_c64(N, w["seed"] + seed_off + i).view(np.float32).reshape(N, 2)).to(dev)
+            for i in range(nin)]
+    nout = 2 if info.plane_bytes * 2 < 20e9 else 1
+    d_out = [torch.empty((info.ntemplates, info.ncols), dtype=torch.float32, device=dev) for _ in range(nout)]
+    with torch.cuda.stream(stream):
+        for i in range(warmup):
+            plan.execute(stream, d_in[i % nin], d_out[i % nout])
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for i in range(steps):
+            plan.execute(stream, d_in[i % nin], d_out[i % nout])
+        e1.record(stream)
+    stream.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    rec = info.as_dict()
+    plan.close()
+    del d_in, d_out
+    torch.cuda.empty_cache()
+    return ms, rec
+
+
+def self_launch(args):
+    """`python bench.py --gpus N` without a torchrun environment: re-execute under torch.distributed.run, one
+    rank per GPU (the driver's own launch line), and pass its exit status on."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
+def plumbing_only(args, w):
+    """--plumbing-only: everything of the N-rank path that is not GPU work (rendezvous, sharding of the job's spectra,
+    barrier, max / sum over ranks, rank 0's JSON line) on the gloo backend: the CPU test of `--gpus N`."""
+    from paper_1804_05335_b200 import dist
+    rank, local_rank, world = dist.init("gloo")
+    lo, hi = dist.shard(w["batch"] * world, rank, world)
+    dist.barrier()
+    t_max = dist.max_over_ranks(1.0 + rank)
+    spectra = dist.sum_over_ranks(hi - lo)
+    if rank == 0:
+        print(json.dumps({"plumbing_only": True, "n_gpus": world, "requested_gpus": args.gpus,
+                          "spectra_per_rank": hi - lo, "spectra_total": int(spectra), "max_over_ranks": t_max,
+                          "config": {"workload": w["name"]}, "scaling": "weak"}))
+    dist.finalize()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=30)
-    ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number 1..5 (default 2: the metric's)")
+    ap.add_argument("--steps", type=int, default=None, help="timed steps (default 20; config 5: 10 steps of 64 launches)")
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=5,
+                    help="BASELINE.json config number 1..5 (default 5: the largest single-GPU workload)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--interbin", type=int, default=None, choices=[0, 1, 2],
                     help="override the config's half-bin mode (0 none, 1 interbinning, 2 two-bin Fourier interpolation)")
-    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-steps", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cufft", action="store_true",
                     help="skip the same-box unfused cuFFT comparator (variant A of the paper, N = 1 only)")
+    ap.add_argument("--no-configs", action="store_true", help="skip the per-config record of configs 2, 3, 4")
     ap.add_argument("--table4", action="store_true",
                     help="sweep the shapes of the paper's Table 4 (n = 2^20..2^23 samples, 65..257 templates) and exit")
+    ap.add_argument("--plumbing-only", action="store_true",
+                    help="run only the multi-rank plumbing (gloo, no GPU work) and print its JSON line")
     args = ap.parse_args()
+    if args.steps is None:
+        args.steps = 10 if args.config == 5 else 20
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
     w = workload(args.config, args.interbin)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        if args.impl == "reference":
+            run_reference(args, w)                      # rank 0 alone runs the reference arm
+            return
+        self_launch(args)
     if args.impl == "reference":
         run_reference(args, w)
+        return
+    if args.plumbing_only:
+        plumbing_only(args, w)
         return
 
     import numpy as np
@@ -355,20 +476,24 @@ def main():
     plan.make_templates()
     info = plan.info
     K, ncols, N = info.ntemplates, info.ncols, info.nbins
+    batch = int(w["batch"])                        # spectra per step per GPU (config 5: 64)
 
-    # inputs: NIN rotating spectra per rank (distinct seeds per rank), resident in HBM before timing;
-    # the plane written each step (>= 713 MB) is far larger than the 126 MB L2.
-    nin = 8
+    # inputs: this rank's shard of the job's batch * world spectra (distinct seeds), resident in HBM before
+    # timing; at least 8 distinct spectra rotate.  The planes written per step (>= 713 MB, 91 GB for config 5)
+    # are far larger than the 126 MB L2; NOUT output planes rotate.
+    lo, hi = dist.shard(batch * world, rank, world)
+    nin = max(8, hi - lo)
     d_in = []
     for i in range(nin):
-        s = synthetic.noise_only_c64(N, w["seed"] + 1000 * rank + i)
+        s = synthetic.noise_only_c64(N, w["seed"] + 1000 * (lo + i))
         d_in.append(torch.from_numpy(s.view(np.float32).reshape(N, 2)).to(dev))
-    nout = 2 if info.plane_bytes * 2 < 40e9 else 1
+    nout = 4 if info.plane_bytes * 4 < 40e9 else 1
     d_out = [torch.empty((K, ncols), dtype=torch.float32, device=dev) for _ in range(nout)]
     stream = torch.cuda.Stream(device=dev)
 
-    def step(i):
-        plan.execute(stream, d_in[i % nin], d_out[i % nout])
+    def step(i):                                   # one step = `batch` launches on one stream, no host sync
+        for b in range(batch):
+            plan.execute(stream, d_in[(i * batch + b) % nin], d_out[(i * batch + b) % nout])
 
     with torch.cuda.stream(stream):
         for i in range(args.warmup):
@@ -380,72 +505,77 @@ def main():
     if rank == 0:
         sampler.start()
         time.sleep(0.3)
-    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     dist.barrier()
     torch.cuda.synchronize()
     launches0 = fdas.fdas_launch_count()
     t_wall0 = time.time()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with torch.cuda.stream(stream):
-        evs[0].record(stream)
+        e0.record(stream)
         for i in range(args.steps):
             step(i)
-            evs[i + 1].record(stream)
+        e1.record(stream)
     stream.synchronize()
     torch.cuda.synchronize()
     t_wall1 = time.time()
     dist.barrier()
     launches = fdas.fdas_launch_count() - launches0
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
-    total_ms = evs[0].elapsed_time(evs[-1])
-    kern_ms = [evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)]   # one launch per step
+    total_ms = e0.elapsed_time(e1)
     total_ms_max = dist.max_over_ranks(total_ms, dev)
-    value = world * args.steps * w["cells"] / (total_ms_max * 1e-3)
+    value = world * args.steps * batch * w["cells"] / (total_ms_max * 1e-3)
+    kernel_ms = total_ms / (args.steps * batch)    # average launch duration over the timed region (this rank)
 
-    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
-    h_in = torch.from_numpy(synthetic.noise_only_c64(N, w["seed"] + 77).view(np.float32).reshape(N, 2)).pin_memory()
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region:
+    # one step = the whole batch through fdas_execute_host (H2D of each spectrum, kernel, D2H of each plane)
+    e2e_steps = args.e2e_steps if args.e2e_steps is not None else (1 if batch > 1 else 3)
+    nh = min(batch, 4)
+    h_in = [torch.from_numpy(synthetic.noise_only_c64(N, w["seed"] + 77 + i).view(np.float32).reshape(N, 2)).pin_memory()
+            for i in range(nh)]
     h_out = torch.empty((K, ncols), dtype=torch.float32).pin_memory()
-    plan.execute_host(stream, h_in, h_out)          # warm-up (allocates the staging buffers)
+    plan.execute_host(stream, h_in[0], h_out)          # warm-up (allocates the staging buffers)
     dist.barrier()
     torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
-    for i in range(args.e2e_steps):
-        plan.execute_host(stream, h_in, h_out)
+    for i in range(e2e_steps):
+        for b in range(batch):
+            plan.execute_host(stream, h_in[b % nh], h_out)
     e1.record(stream)
     stream.synchronize()
     e2e_ms = dist.max_over_ranks(e0.elapsed_time(e1), dev)
-    e2e_value = world * args.e2e_steps * w["cells"] / (e2e_ms * 1e-3)
+    e2e_value = world * e2e_steps * batch * w["cells"] / (e2e_ms * 1e-3)
     checksum = float(h_out[K // 2, : min(1024, ncols)].sum())
 
     # ---- threshold-search mode: the same fused kernel with a candidate
-    # sink instead of the plane store; reported beside the headline, never instead of it
+    # sink instead of the plane store; reported beside the headline, never instead of it (per spectrum)
     thr_val, thr_cap = 16.0, 1 << 20
     d_cands = torch.empty(thr_cap * 16, dtype=torch.uint8, device=dev)
     d_count = torch.zeros(1, dtype=torch.int64, device=dev)
     h_cands = torch.empty(thr_cap * 16, dtype=torch.uint8).pin_memory()
     h_count = torch.zeros(1, dtype=torch.int64).pin_memory()
+    thr_steps = 20
     with torch.cuda.stream(stream):
         for i in range(3):
             plan.execute_threshold(stream, d_in[i % nin], thr_val, d_cands, thr_cap, d_count)
         t0e, t1e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         t0e.record(stream)
-        for i in range(args.steps):
+        for i in range(thr_steps):
             plan.execute_threshold(stream, d_in[i % nin], thr_val, d_cands, thr_cap, d_count)
         t1e.record(stream)
     stream.synchronize()
-    thr_ms = dist.max_over_ranks(t0e.elapsed_time(t1e), dev) / args.steps
-    plan.execute_threshold_host(stream, h_in, thr_val, h_cands, thr_cap, h_count)      # warm-up (staging)
+    thr_ms = dist.max_over_ranks(t0e.elapsed_time(t1e), dev) / thr_steps
+    plan.execute_threshold_host(stream, h_in[0], thr_val, h_cands, thr_cap, h_count)      # warm-up (staging)
     t0e.record(stream)
-    for i in range(args.e2e_steps):
-        plan.execute_threshold_host(stream, h_in, thr_val, h_cands, thr_cap, h_count)
+    for i in range(3):
+        plan.execute_threshold_host(stream, h_in[i % nh], thr_val, h_cands, thr_cap, h_count)
     t1e.record(stream)
     stream.synchronize()
-    thr_e2e_ms = dist.max_over_ranks(t0e.elapsed_time(t1e), dev) / args.e2e_steps
+    thr_e2e_ms = dist.max_over_ranks(t0e.elapsed_time(t1e), dev) / 3
     thr_found = int(h_count.item())
 
     fp32_probe = fdas.fdas_measure_fp32_peak(stream, 4000) if rank == 0 else None
 
-    # ---- same-box comparator: the paper's unfused cuFFT pipeline (harness-side, N = 1 only)
+    # ---- same-box comparator: the paper's unfused cuFFT pipeline (harness-side, N = 1 only, one spectrum)
     cufft_ms, cufft_err = None, None
     if world == 1 and not args.no_cufft:
         del h_out
@@ -453,59 +583,73 @@ def main():
             cufft_ms = time_cufft(torch, plan, dev, d_in[0], d_out[0])
         except Exception as exc:                      # a comparator failure must not cost the bench line
             cufft_err = f"{type(exc).__name__}: {exc}"[:200]
+    plan_rec = info.as_dict()
+    plane_bytes = info.plane_bytes
+    plan.close()
+    del d_in, d_out, d_cands
+    torch.cuda.empty_cache()
+
+    # ---- the other full-size configs of BASELINE.json in the same line (rank 0's GPU, one spectrum per launch)
+    sm_max_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
+    others = {}
+    if rank == 0 and not args.no_configs and args.interbin is None:
+        for c in (2, 3, 4, 5):
+            if c == args.config:
+                continue
+            wc = workload(c)
+            try:
+                ms, rec = time_config(torch, fdas, synthetic, dev, stream, wc, 20, 3)
+            except Exception as exc:
+                others[wc["name"]] = {"unavailable": f"{type(exc).__name__}: {exc}"[:200]}
+                continue
+            rc = roofline_record(wc, info, ms, peaks, sm_max_mhz, c, False)
+            other = rc["hbm"] or rc["alu"]
+            others[wc["name"]] = {
+                "kernel_ms_per_spectrum": ms, "value": wc["cells"] / (ms * 1e-3), "unit": UNIT,
+                "bins_per_s": wc["nbins"] / (ms * 1e-3), "bound": rc["bound"], "frac": rc["frac"],
+                "frac_hbm": rc["frac"] if rc["bound"] == "hbm" else other["frac"],
+                "frac_alu": rc["frac"] if rc["bound"] == "alu" else other["frac"],
+                "achieved_gbs": wc["alg_bytes"] / (ms * 1e-3) / 1e9, "achieved_tflops": wc["alg_flops"] / (ms * 1e-3) / 1e12,
+                "traffic": rc["traffic"], "traffic_source": rc["traffic_source"], "kernel": rc["kernel"],
+                "templates": wc["K"], "nbins": wc["nbins"], "seglen": wc["seglen"], "interbin": wc["interbin"],
+                "ctas_per_sm": rec["ctas_per_sm"], "regs": rec["regs"]}
+    dist.barrier()
 
     if rank == 0:
-        avg_kernel_s = (sum(kern_ms) / len(kern_ms)) * 1e-3
-        sm_max_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
-        fp32_peak = info.sm_count * 128 * 2 * sm_max_mhz * 1e6 / 1e12
-        t_hbm = w["alg_bytes"] / (peaks["hbm_gbs"] * 1e9)
-        t_alu = w["alg_flops"] / (fp32_peak * 1e12)
-        ach_gbs = w["alg_bytes"] / avg_kernel_s / 1e9
-        ach_tf = w["alg_flops"] / avg_kernel_s / 1e12
-        traffic = NCU_TRAFFIC_BYTES.get(args.config) if args.interbin is None else None if args.interbin is None else None
-        hbm = {"bound": "hbm", "achieved": ach_gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-               "frac": ach_gbs / peaks["hbm_gbs"], "traffic": traffic, "peak_source": peaks["source"]}
-        alu = {"bound": "alu", "achieved": ach_tf, "peak": fp32_peak, "unit": "TFLOP/s",
-               "frac": ach_tf / fp32_peak, "traffic": traffic,
-               "peak_source": f"{info.sm_count} SMs x 128 FP32 lanes x 2 x {sm_max_mhz:.0f} MHz (DESIGN.md)",
-               "fma_probe_tflops": fp32_probe}
-        roof = dict(alu if t_alu >= t_hbm else hbm)      # north_star: the slower bound is the roofline
-        roof.update(kernel={8192: "fdas_fused_kernel_8k", 4096: "fdas_fused_kernel2"}.get(w["seglen"], "fdas_fused_kernel"),
-                    traffic_source="ncu --set full, profiles/%s (bytes per launch)" % NCU_TRAFFIC_FILE[args.config]
-                    if traffic else None, kernel_ms=avg_kernel_s * 1e3,
-                    alg_bytes=w["alg_bytes"], alg_flops=w["alg_flops"],
-                    t_bound_ms={"hbm": t_hbm * 1e3, "alu": t_alu * 1e3},
-                    hbm=hbm if roof["bound"] == "alu" else None, alu=alu if roof["bound"] == "hbm" else None)
+        roof = roofline_record(w, info, kernel_ms, peaks, sm_max_mhz, args.config, args.interbin is not None, fp32_probe)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms_max / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": w["name"], "nbins": N, "templates": K, "zmax": w["zmax"], "dz": w["dz"],
-                       "seglen": w["seglen"], "interbin": w["interbin"], "spectra_per_step_per_gpu": 1,
-                       "l2": f"plane written per step = {info.plane_bytes / 1e6:.0f} MB > 126 MB L2; "
-                             f"{nin} rotating input spectra ({nin * 8 * N / 1e6:.0f} MB)",
-                       "grid": info.grid, "threads": info.threads, "ctas_per_sm": info.ctas_per_sm,
-                       "regs": info.regs, "smem_bytes": info.smem_bytes, "overlap": info.overlap,
-                       "useful": info.useful, "nseg": info.nseg},
-            "bins_per_s": world * args.steps * N / (total_ms_max * 1e-3),
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * N,
-                    "d2h_bytes_per_step": info.plane_bytes, "steps": args.e2e_steps,
-                    "ms_per_step": e2e_ms / args.e2e_steps, "checksum": checksum},
+                       "seglen": w["seglen"], "interbin": w["interbin"], "spectra_per_step_per_gpu": batch,
+                       "launches_per_step": batch,
+                       "l2": f"planes written per step = {batch * plane_bytes / 1e6:.0f} MB > 126 MB L2; "
+                             f"{nin} distinct input spectra ({nin * 8 * N / 1e6:.0f} MB), {nout} rotating output planes",
+                       "grid": plan_rec["grid"], "threads": plan_rec["threads"], "ctas_per_sm": plan_rec["ctas_per_sm"],
+                       "regs": plan_rec["regs"], "smem_bytes": plan_rec["smem_bytes"], "overlap": plan_rec["overlap"],
+                       "useful": plan_rec["useful"], "nseg": plan_rec["nseg"]},
+            "bins_per_s": world * args.steps * batch * N / (total_ms_max * 1e-3),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": batch * 8 * N,
+                    "d2h_bytes_per_step": batch * plane_bytes, "steps": e2e_steps,
+                    "ms_per_step": e2e_ms / e2e_steps, "checksum": checksum},
             "gpu_launches": launches,
             "clocks": clocks,
             "roofline": roof,
         }
+        if others:
+            out["configs"] = others
         out["threshold_search"] = {
             "what": "fdas_execute_threshold: same fused kernel, cells with P > threshold appended to a candidate "
-                    "list instead of the plane store (paper's stated next step, PAPER.md:73, :331)",
-            "threshold": thr_val, "candidates_found": thr_found, "ms_per_step": thr_ms,
+                    "list instead of the plane store (paper's stated next step, PAPER.md:73, :331); per spectrum",
+            "threshold": thr_val, "candidates_found": thr_found, "ms_per_spectrum": thr_ms,
             "value": world * w["cells"] / (thr_ms * 1e-3), "unit": "cells searched/s",
             "e2e": {"value": world * w["cells"] / (thr_e2e_ms * 1e-3), "unit": "cells searched/s",
-                    "ms_per_step": thr_e2e_ms, "h2d_bytes_per_step": 8 * N,
-                    "d2h_bytes_per_step": 8 + 16 * min(thr_found, thr_cap)}}
+                    "ms_per_spectrum": thr_e2e_ms, "h2d_bytes_per_spectrum": 8 * N,
+                    "d2h_bytes_per_spectrum": 8 + 16 * min(thr_found, thr_cap)}}
         if cufft_ms is not None:
-            out["cufft_unfused"] = {"ms_per_step": cufft_ms, "value": w["cells"] / (cufft_ms * 1e-3), "unit": UNIT,
-                                    "fused_speedup": cufft_ms / (avg_kernel_s * 1e3),
+            out["cufft_unfused"] = {"ms_per_spectrum": cufft_ms, "value": w["cells"] / (cufft_ms * 1e-3), "unit": UNIT,
+                                    "fused_speedup": cufft_ms / kernel_ms,
                                     "what": "paper's variant A on this GPU (PAPER.md:101-119): segment copy, torch.fft "
                                             "(cuFFT) forward, broadcast multiply, cuFFT inverse, discard + power; "
                                             "context for the paper's custom-vs-cuFFT ratio (PAPER.md:237), not a target"}
@@ -514,7 +658,6 @@ def main():
         if not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(w)
         print(json.dumps(out))
-    plan.close()
     dist.finalize()
 
 

@@ -47,7 +47,9 @@ def bank_z(zmax: float, dz: float) -> np.ndarray:
     nhalf = int(round(zmax / dz))
     if abs(nhalf * dz - zmax) > 1e-9 * max(1.0, abs(zmax)):
         raise ValueError("zmax/dz must be an integer")
-    return np.array([-zmax + k * dz for k in range(2 * nhalf + 1)], dtype=np.float64)
+    zs = np.array([-zmax + k * dz for k in range(2 * nhalf + 1)], dtype=np.float64)
+    zs[nhalf] = 0.0                      # the centre template is z = 0 exactly, also for a fractional dz
+    return zs
 
 
 def halfwidth(z: float) -> int:

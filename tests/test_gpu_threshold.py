@@ -165,3 +165,30 @@ def test_threshold_host_end_to_end():
         rec = h_cands.numpy().view(fd.CANDIDATE_DTYPE)[:count_d]
         rec = rec[np.lexsort((rec["col"], rec["row"]))]
         assert np.array_equal(rec, rec_d)
+
+
+def test_execute_host_after_threshold_host_on_the_same_plan():
+    """The host entry points share the input staging buffer but allocate their output staging independently:
+    a plan whose first host call was the threshold search must still serve fdas_execute_host."""
+    import torch
+    from oracle import fdas_oracle as orc
+    from paper_1804_05335_b200 import fdas as fd, synthetic as syn
+    n, cap = 30000, 1 << 12
+    spec = syn.make_spectrum(n, 99, [(0.5 * n, 6.0, 12.0)])
+    with fd.Plan(n, 20.0, 2.0, 1024, 1) as plan:
+        plan.make_templates()
+        h_spec = torch.from_numpy(spec.view(np.float32).reshape(n, 2)).pin_memory()
+        h_cands = torch.zeros(cap * 16, dtype=torch.uint8).pin_memory()
+        h_count = torch.zeros(1, dtype=torch.int64).pin_memory()
+        st = torch.cuda.current_stream()
+        plan.execute_threshold_host(st, h_spec, 12.0, h_cands, cap, h_count)
+        first = int(h_count.item())
+        h_plane = torch.full((21, 2 * n), float("nan"), dtype=torch.float32).pin_memory()
+        plan.execute_host(st, h_spec, h_plane)                     # used to return FDAS_ERR_INVALID_ARG
+        plane = h_plane.numpy().astype(np.float64)
+        assert np.all(np.isfinite(plane))
+        for k in (0, 10, 13, 20):
+            ref = orc.plane_row(spec, orc.bank_z(20.0, 2.0)[k], True)
+            assert np.max(np.abs(plane[k] - ref)) <= 1e-4 * np.max(ref)
+        plan.execute_threshold_host(st, h_spec, 12.0, h_cands, cap, h_count)
+        assert int(h_count.item()) == first == int(np.count_nonzero(h_plane.numpy() > 12.0))

@@ -384,3 +384,36 @@ def test_p12_half_bin_chirp_peaks_in_its_odd_column():
     b = syn.make_spectrum(1 << 16, 34)
     p = orc.plane_row(b, z0, 2)
     assert abs(np.mean(p[1::2]) - e) < 12.0 / math.sqrt(b.size)
+
+
+def test_p12_sampled_cells_of_the_two_bin_plane_are_the_literal_interleaved_sum():
+    """`plane_cells(..., interbin=2)` (sampled checks of the GPU's interbin = 2 planes): column c of the
+    double-resolution plane written out as a literal loop over the ZERO-INTERLEAVED spectrum and
+    the half-spaced template h_z(j/2) -- even and odd columns, both edges, z of both signs and z = 0 (whose odd
+    columns are the zero-padded-DFT interpolation of P12's second pin)."""
+    a = syn.make_spectrum(300, 13, [(140.5, 5.0, 8.0)])
+    a128 = a.astype(np.complex128)
+    cols = np.array([0, 1, 2, 3, 279, 280, 281, 598, 599])
+    for z in (0.0, 6.0, -20.0):
+        m = orc.halfwidth(z)
+        t = orc.response(z, 0.5 * np.arange(-2 * m, 2 * m + 1))      # h_z(j/2), j = -2m..2m
+        ref = np.zeros(cols.size)
+        for i, c in enumerate(cols):
+            acc = 0j
+            for j in range(-2 * m, 2 * m + 1):
+                q = c + j                                            # index in the interleaved spectrum
+                if 0 <= q < 600 and q % 2 == 0:                      # odd entries are the interleaved zeros
+                    acc += a128[q // 2] * np.conj(t[j + 2 * m])
+            ref[i] = acc.real ** 2 + acc.imag ** 2
+        got = orc.plane_cells(a, z, cols, 2)
+        assert np.max(np.abs(got - ref)) < 1e-12 * max(1.0, ref.max())
+        assert np.max(np.abs(got - orc.plane_row(a, z, 2)[cols])) < 1e-12 * max(1.0, ref.max())
+    # even columns are the plain plane's cells
+    assert np.allclose(orc.plane_cells(a, 6.0, cols[cols % 2 == 0], 2), orc.plane_cells(a, 6.0, cols[cols % 2 == 0] // 2, False),
+                       rtol=1e-12, atol=1e-15)
+
+
+def test_bank_centre_is_exactly_zero_for_fractional_dz():
+    for zmax, dz in ((6.0, 0.5), (0.3, 0.1), (84.0, 2.0), (2.1, 0.7)):
+        zs = orc.bank_z(zmax, dz)
+        assert zs[zs.size // 2] == 0.0 and np.all(np.diff(zs) > 0)

@@ -422,7 +422,7 @@ def plumbing_only(args, w):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=None, help="timed steps (default 20; config 5: 10 steps of 64 launches)")
+    ap.add_argument("--steps", type=int, default=None, help="timed steps (default 20; config 5: each step is 64 launches)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=5,
                     help="BASELINE.json config number 1..5 (default 5: the largest single-GPU workload)")
@@ -440,7 +440,7 @@ def main():
                     help="run only the multi-rank plumbing (gloo, no GPU work) and print its JSON line")
     args = ap.parse_args()
     if args.steps is None:
-        args.steps = 10 if args.config == 5 else 20
+        args.steps = 20
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
     w = workload(args.config, args.interbin)

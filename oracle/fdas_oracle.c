@@ -61,6 +61,38 @@ void fdas_oracle_correlate_at(const float *A, int64_t N, const double *h, int32_
         correlate_one(A, N, h, m, cols[i], &y[2 * i], &y[2 * i + 1]);
 }
 
+/*
+ * Discrete Fourier transform of a REAL time series, eq. 5 written out:
+ *
+ *     X[k] = sum_{j=0}^{n-1} x[j] exp(-2 pi i j k / n)          (unnormalised, forward sign)
+ *
+ * at the listed bins k (any integers; the sum is the definition, so bins >= n/2 are allowed and give the
+ * conjugate-symmetric half).  This is the "long real-to-complex FFT" in front of the correlations
+ * (PAPER.md:79 Fig. 2, :105 "cuFFT R2C", :190, :219), evaluated directly: O(n) per bin, the phase
+ * reduced exactly in integers (j k mod n) before the one sincos per term.  x: n float32 samples (the values
+ * the GPU receives, up-converted); out: interleaved (re, im) doubles.
+ */
+#include <math.h>
+void fdas_oracle_dft_real_at(const float *x, int64_t n, const int64_t *bins, int64_t nb, double *out)
+{
+    const double w = -2.0 * 3.14159265358979323846264338327950288 / (double)n;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t b = 0; b < nb; ++b) {
+        const int64_t k = ((bins[b] % n) + n) % n;
+        double sr = 0.0, si = 0.0;
+        int64_t ph = 0;                              /* (j k) mod n, advanced by k per sample */
+        for (int64_t j = 0; j < n; ++j) {
+            const double a = w * (double)ph;
+            sr += (double)x[j] * cos(a);
+            si += (double)x[j] * sin(a);
+            ph += k;
+            if (ph >= n) ph -= n;
+        }
+        out[2 * b] = sr;
+        out[2 * b + 1] = si;
+    }
+}
+
 int32_t fdas_oracle_threads(void)
 {
 #ifdef _OPENMP

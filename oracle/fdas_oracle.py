@@ -25,6 +25,15 @@ and a pure-Python triple loop on tiny inputs; the threshold search (`candidates`
 exponential tail law of noise powers, the 0 / +inf thresholds and an injected chirp's cell; the
 2-bin Fourier interpolation (`interbin = 2`) by a brute-force DFT of a time series zero-padded to
 twice its length, a half-bin tone's full recovery and the time-domain chirp at a half-integer centre.
+  * the real-to-complex transform in front of the correlations: eq. 5
+    summed directly for a real series, `dft_real_at` / `dft_real` (reading R17),
+  * harmonic summing of the plane (reading R18), `harmonic_sum` /
+    `harmonic_candidates`.
+
+More pins: `dft_real*` by a literal O(n^2) Python loop, a pure tone's bin and amplitude, Parseval, conjugate
+symmetry, linearity, the shift theorem and numpy's rfft as a third opinion; `harmonic_sum` by literal loops on a
+tiny plane, the identity at one harmonic, a time-domain signal with power in harmonics 1, 2 and 4 peaking at the
+fundamental's cell, and the Erlang tail law of summed noise powers.
 No function here is "parity unpinned".
 """
 from __future__ import annotations
@@ -119,6 +128,8 @@ def _load():
         lib.fdas_oracle_correlate_at.argtypes = [vp, i64, vp, i32, vp, i64, vp]
         lib.fdas_oracle_correlate_at.restype = None
         lib.fdas_oracle_threads.restype = i32
+        lib.fdas_oracle_dft_real_at.argtypes = [vp, i64, vp, i64, vp]
+        lib.fdas_oracle_dft_real_at.restype = None
         _lib = lib
     return _lib
 
@@ -284,3 +295,70 @@ def candidates(spectrum, zmax: float, dz: float, threshold: float, interbin=Fals
 def cmacs(n: int, zmax: float, dz: float) -> int:
     """Complex multiply-accumulates of the direct sum for one spectrum: N * sum_z (2 m_z + 1)."""
     return int(n) * int(sum(2 * halfwidth(z) + 1 for z in bank_z(zmax, dz)))
+
+
+# --------------------------------------------------------------------------------------
+# the real-to-complex transform in front of the correlations (SURVEY.md section 8(f) F3)
+# --------------------------------------------------------------------------------------
+
+def dft_real_at(x, bins) -> np.ndarray:
+    """X[k] = sum_j x[j] exp(-2 pi i j k / n) (eq. 5; unnormalised) of the REAL series x (float32
+    samples, up-converted) at the listed bins, by direct summation in C (O(n) per bin)."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    if x.ndim != 1:
+        raise ValueError("time series must be 1-D")
+    bins = np.ascontiguousarray(bins, dtype=np.int64)
+    out = np.empty(bins.size, dtype=np.complex128)
+    _load().fdas_oracle_dft_real_at(x.ctypes.data, x.size, bins.ctypes.data, bins.size, out.ctypes.data)
+    return out
+
+
+def dft_real(x) -> np.ndarray:
+    """The spectrum the correlations take (reading R17): bins k = 0 .. n/2 - 1 of the real series'
+    DFT (DC kept, the Nyquist bin dropped), unnormalised.  O(n^2): small n only."""
+    n = np.asarray(x).size
+    if n % 2:
+        raise ValueError("even number of samples")
+    return dft_real_at(x, np.arange(n // 2))
+
+
+# --------------------------------------------------------------------------------------
+# harmonic summing (SURVEY.md section 8(f) F2, PAPER.md:73, :79, :331; DESIGN.md reading R18)
+# --------------------------------------------------------------------------------------
+
+def harmonic_rows(zmax: float, dz: float, nharm: int) -> np.ndarray:
+    """Rows k of the bank whose harmonics h z_k, h = 1..nharm, all lie inside the bank (|z_k| <= zmax / nharm)."""
+    zs = bank_z(zmax, dz)
+    nhalf = (zs.size - 1) // 2
+    lim = nhalf // int(nharm)
+    return np.arange(nhalf - lim, nhalf + lim + 1)
+
+
+def harmonic_sum(plane: np.ndarray, zmax: float, dz: float, nharm: int) -> np.ndarray:
+    """
+    S_H[k][c] = sum_{h=1}^{H} P[row(h z_k)][h c]: a signal whose fundamental sits at column c with drift z_k has its
+    h-th harmonic at column h c with drift h z_k (frequency AND frequency derivative scale with h), so its power is
+    collected at the fundamental's cell.  Defined for the rows of `harmonic_rows` and the columns c with
+    H c <= ncols - 1; returned as a (rows, ceil(ncols / H)) float64 array, row i <-> bank row harmonic_rows()[i].
+    """
+    p = np.asarray(plane, dtype=np.float64)
+    k_all, ncols = p.shape
+    nharm = int(nharm)
+    rows = harmonic_rows(zmax, dz, nharm)
+    nhalf = (k_all - 1) // 2
+    nc = (ncols - 1) // nharm + 1
+    out = np.zeros((rows.size, nc), dtype=np.float64)
+    for i, k in enumerate(rows):
+        for h in range(1, nharm + 1):
+            kh = nhalf + h * (int(k) - nhalf)          # row of h z_k
+            out[i] += p[kh, 0:h * (nc - 1) + 1:h]
+    return out
+
+
+def harmonic_candidates(plane: np.ndarray, zmax: float, dz: float, nharm: int, threshold: float):
+    """Cells of the H-harmonic sum above the threshold (strict): (bank row k, fundamental column c, S) sorted by
+    (row, column)."""
+    s = harmonic_sum(plane, zmax, dz, nharm)
+    rows = harmonic_rows(zmax, dz, nharm)
+    i, c = np.nonzero(s > threshold)
+    return rows[i].astype(np.int64), c.astype(np.int64), s[i, c]

@@ -154,8 +154,56 @@ fdas_status fdas_execute_threshold(fdas_plan *plan, void *stream, const void *d_
 fdas_status fdas_execute_threshold_host(fdas_plan *plan, void *stream, const void *h_spectrum, float threshold,
                                         fdas_candidate *h_cands, int64_t capacity, uint64_t *h_count);
 
+/*
+ * Harmonic summing of a stored plane with a threshold search on the sums ("harmonic summing",
+ * :79 Fig. 2, :331; reading R18).  A signal whose fundamental sits at plane column c with drift z_k has
+ * its h-th harmonic at column h*c with drift h*z_k, so
+ *     S_H[k][c] = sum_{h=1}^{H} P[row(h z_k)][h c]
+ * is formed for the rows with |z_k| <= zmax / H (all H harmonics inside the bank) and the columns with
+ * H*c <= ncols - 1, and every cell with S_H > threshold (strict) is appended to `d_cands` as
+ * {col = c, row = k (bank row of the fundamental), power = S_H}.  nharm = 1 is the plain threshold search of a
+ * stored plane.  One launch on `stream`; allocates nothing, never synchronises the host.
+ *   d_plane : device, the ntemplates x ncols float32 plane fdas_execute wrote (read only), 16-byte aligned.
+ *   nharm   : H >= 1 (searches usually sum 2, 4, 8, 16 harmonics in turn; call once per H).
+ *   d_cands / capacity / d_count : as for fdas_execute_threshold (d_count is zeroed on `stream` first).
+ * Errors: FDAS_ERR_INVALID_ARG (null pointers, nharm < 1, NaN threshold, capacity < 0), FDAS_ERR_ALIGNMENT,
+ * FDAS_ERR_CUDA.  Needs no templates (works on any plane of the plan's shape).
+ */
+fdas_status fdas_harmonic_sum_threshold(fdas_plan *plan, void *stream, const float *d_plane, int32_t nharm,
+                                        float threshold, fdas_candidate *d_cands, int64_t capacity,
+                                        uint64_t *d_count);
+
 /* Free the plan and everything it owns.  fdas_destroy(NULL) is a no-op returning FDAS_OK. */
 fdas_status fdas_destroy(fdas_plan *plan);
+
+/* ---- the real-to-complex transform in front of the correlations ---- */
+
+typedef struct fdas_r2c_plan fdas_r2c_plan; /* opaque; created/destroyed by the library */
+
+/*
+ * Plan the transform of a REAL time series of `nsamples` float32 samples into the nsamples/2 complex64 bins the
+ * correlations take (PAPER.md:79 Fig. 2, :105 "cuFFT R2C", :190, :219; eq. 5; reading R17):
+ *     X[k] = scale * sum_j x[j] exp(-2 pi i j k / nsamples),  k = 0 .. nsamples/2 - 1
+ * (DC kept, the Nyquist bin dropped).  nsamples must be a power of two, 2^10 <= nsamples <= 2^25
+ * (FDAS_ERR_UNSUPPORTED otherwise).  Allocates a work array of nsamples/2 complex64 and the twiddle tables
+ * on the current device and fills the tables (synchronises once).
+ */
+fdas_status fdas_r2c_plan_create(fdas_r2c_plan **out, int64_t nsamples);
+
+/*
+ * Transform one series: three launches on `stream` (column transforms, row transforms, untangle), no host
+ * synchronisation, no allocation.
+ *   d_timeseries : device, nsamples float32, 8-byte aligned; read only.
+ *   d_spectrum   : device, nsamples/2 x {float re, float im}, 16-byte aligned; every bin is written.  It can be
+ *                  handed to fdas_execute of a plan with nbins = nsamples/2 on the same stream.
+ *   scale        : multiplies every bin (1/nsamples-type normalisations are the caller's choice; the paper's
+ *                  pipeline normalises the spectrum outside the part it covers).
+ */
+fdas_status fdas_r2c_execute(fdas_r2c_plan *plan, void *stream, const float *d_timeseries, void *d_spectrum,
+                             float scale);
+
+/* Free the plan.  fdas_r2c_destroy(NULL) is a no-op returning FDAS_OK. */
+fdas_status fdas_r2c_destroy(fdas_r2c_plan *plan);
 
 /* ---- introspection for harnesses and tests (not on the hot path) ---- */
 

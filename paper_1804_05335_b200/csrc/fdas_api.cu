@@ -428,6 +428,26 @@ fdas_status fdas_execute_threshold_host(fdas_plan *p, void *stream, const void *
     return FDAS_OK;
 }
 
+fdas_status fdas_harmonic_sum_threshold(fdas_plan *p, void *stream, const float *d_plane, int32_t nharm,
+                                        float threshold, fdas_candidate *d_cands, int64_t capacity, uint64_t *d_count)
+{
+    if (!p || !d_plane || !d_count || nharm < 1 || capacity < 0 || (capacity > 0 && !d_cands) ||
+        threshold != threshold || !on_plan_device(p))
+        return FDAS_ERR_INVALID_ARG;
+    if (((uintptr_t)d_plane & 15) || ((uintptr_t)d_cands & 15) || ((uintptr_t)d_count & 7)) return FDAS_ERR_ALIGNMENT;
+    const fdas_info &I = p->info;
+    cudaStream_t st = (cudaStream_t)stream;
+    FDAS_CUDA(p, cudaMemsetAsync(d_count, 0, sizeof(uint64_t), st));
+    const int nhalf = (I.ntemplates - 1) / 2, lim = nhalf / nharm;      // rows |z_k| <= zmax / H
+    const long long nc = (I.ncols - 1) / nharm + 1;
+    const dim3 grid((unsigned)((nc + 255) / 256), (unsigned)(2 * lim + 1));
+    harmonic_sum_kernel<<<grid, 256, 0, st>>>(d_plane, I.ncols, I.ntemplates, nharm, nhalf - lim, threshold,
+                                              (Candidate *)d_cands, capacity, (unsigned long long *)d_count);
+    g_launches += 1;
+    FDAS_CUDA(p, cudaGetLastError());
+    return FDAS_OK;
+}
+
 fdas_status fdas_destroy(fdas_plan *p)
 {
     if (!p) return FDAS_OK;
@@ -489,6 +509,116 @@ fdas_status fdas_get_template_spectrum(fdas_plan *p, int32_t k, float *host_re_i
         host_re_im[2 * f] = v.x;
         host_re_im[2 * f + 1] = conj ? -v.y : v.y; // H_{+z} = conj(H_{-z})
     }
+    return FDAS_OK;
+}
+
+// ---------------------------------------------------------------- real-to-complex transform (fdas_r2c.cuh)
+} // extern "C"
+
+struct fdas_r2c_plan {
+    int64_t n, M;
+    int device, M1, M2, log2M1, log2M2, tile1, tile2;
+    float2 *d_work, *d_w1, *d_w2, *d_tlo, *d_thi;
+};
+
+extern "C" {
+
+fdas_status fdas_r2c_plan_create(fdas_r2c_plan **out, int64_t nsamples)
+{
+    if (!out) return FDAS_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (nsamples <= 0) return FDAS_ERR_INVALID_ARG;
+    int p2 = 0;
+    while ((1ll << p2) < nsamples) ++p2;
+    if ((1ll << p2) != nsamples || p2 < 10 || p2 > 25) return FDAS_ERR_UNSUPPORTED;
+    fdas_r2c_plan *p = new (std::nothrow) fdas_r2c_plan();
+    if (!p) return FDAS_ERR_NOMEM;
+    std::memset(p, 0, sizeof(*p));
+    p->n = nsamples;
+    p->M = nsamples / 2;
+    p->log2M1 = (p2 - 1) / 2;
+    p->log2M2 = (p2 - 1) - p->log2M1;
+    p->M1 = 1 << p->log2M1;
+    p->M2 = 1 << p->log2M2;
+    auto tile_for = [](int R, int other) {          // transforms per CTA: <= 16384 points, <= 32, <= what exists
+        int t = 16384 / R;
+        if (t > 32) t = 32;
+        if (t > other) t = other;
+        return t;
+    };
+    p->tile1 = tile_for(p->M1, p->M2);
+    p->tile2 = tile_for(p->M2, p->M1);
+    g_create_err[0] = 0;
+    const int64_t nhi = (nsamples + 4095) / 4096;
+    cudaError_t e = cudaGetDevice(&p->device);
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_work, (size_t)p->M * sizeof(float2));
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_w1, (size_t)p->M1 * sizeof(float2));
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_w2, (size_t)p->M2 * sizeof(float2));
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_tlo, 4096 * sizeof(float2));
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_thi, (size_t)nhi * sizeof(float2));
+    if (e == cudaSuccess) {
+        r2c_table_kernel<<<(p->M1 + 127) / 128, 128>>>(p->d_w1, p->M1, 1, p->M1);
+        r2c_table_kernel<<<(p->M2 + 127) / 128, 128>>>(p->d_w2, p->M2, 1, p->M2);
+        r2c_table_kernel<<<32, 128>>>(p->d_tlo, 4096, 1, nsamples);
+        r2c_table_kernel<<<(unsigned)((nhi + 127) / 128), 128>>>(p->d_thi, nhi, 4096, nsamples);
+        g_launches += 4;
+        e = cudaDeviceSynchronize();
+    }
+    for (const void *k : {(const void *)r2c_pass1_kernel, (const void *)r2c_pass2_kernel})
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (16384 + 32) * 8);
+    if (e != cudaSuccess) {
+        snprintf(g_create_err, sizeof(g_create_err), "fdas_r2c_plan_create: %s", cudaGetErrorString(e));
+        const bool nomem = e == cudaErrorMemoryAllocation;
+        cudaGetLastError();
+        fdas_r2c_destroy(p);
+        return nomem ? FDAS_ERR_NOMEM : FDAS_ERR_CUDA;
+    }
+    *out = p;
+    return FDAS_OK;
+}
+
+fdas_status fdas_r2c_execute(fdas_r2c_plan *p, void *stream, const float *d_timeseries, void *d_spectrum, float scale)
+{
+    if (!p || !d_timeseries || !d_spectrum) return FDAS_ERR_INVALID_ARG;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device) return FDAS_ERR_INVALID_ARG;
+    if (((uintptr_t)d_timeseries & 7) || ((uintptr_t)d_spectrum & 15)) return FDAS_ERR_ALIGNMENT;
+    cudaStream_t st = (cudaStream_t)stream;
+    R2CParams q;
+    q.tlo = p->d_tlo;
+    q.thi = p->d_thi;
+    q.M = p->M;
+    q.M1 = p->M1;
+    q.M2 = p->M2;
+    q.scale = scale;
+    q.in = (const float2 *)d_timeseries;
+    q.out = p->d_work;
+    q.wR = p->d_w1;
+    q.log2R = p->log2M1;
+    q.tile = p->tile1;
+    r2c_pass1_kernel<<<p->M2 / p->tile1, 256, (size_t)p->tile1 * (p->M1 + 1) * sizeof(float2), st>>>(q);
+    q.in = p->d_work;
+    q.out = (float2 *)d_spectrum;
+    q.wR = p->d_w2;
+    q.log2R = p->log2M2;
+    q.tile = p->tile2;
+    r2c_pass2_kernel<<<p->M1 / p->tile2, 256, (size_t)p->tile2 * (p->M2 + 1) * sizeof(float2), st>>>(q);
+    r2c_untangle_kernel<<<(unsigned)((p->M / 2 + 1 + 255) / 256), 256, 0, st>>>(q);
+    g_launches += 3;
+    if (cudaGetLastError() != cudaSuccess) return FDAS_ERR_CUDA;
+    return FDAS_OK;
+}
+
+fdas_status fdas_r2c_destroy(fdas_r2c_plan *p)
+{
+    if (!p) return FDAS_OK;
+    cudaFree(p->d_work);
+    cudaFree(p->d_w1);
+    cudaFree(p->d_w2);
+    cudaFree(p->d_tlo);
+    cudaFree(p->d_thi);
+    cudaGetLastError();
+    delete p;
     return FDAS_OK;
 }
 

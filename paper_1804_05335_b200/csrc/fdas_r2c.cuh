@@ -1,0 +1,160 @@
+// Real-to-complex transform of the time series in front of the correlations.
+//
+// PAPER.md:79 (Fig. 2: the FDAS pipeline starts from the FFT of the time series), :105 ("cuFFT R2C"), :190 and
+// :219 (the long real FFT is inside every timing of the paper), eq. 5:
+//
+//     X[k] = scale * sum_{j=0}^{n-1} x[j] exp(-2 pi i j k / n),   k = 0 .. n/2 - 1     (reading R17: DC kept,
+//                                                                                       Nyquist bin dropped)
+// n = 2^p real samples.  The series is read as M = n/2 complex numbers z[j] = x[2j] + i x[2j+1]; Z = DFT_M(z) by the
+// four-step decomposition M = M1 * M2 (j = j1 M2 + j2, k = k1 + M1 k2), two passes through HBM:
+//
+//   pass 1  one CTA per tile of adjacent columns j2: length-M1 transforms over j1 in shared memory,
+//           times exp(-2 pi i j2 k1 / M), stored at [k1][j2]                      (plan-owned work array)
+//   pass 2  one CTA per tile of adjacent rows k1: length-M2 transforms over j2 in shared memory, stored
+//           transposed at k = k1 + M1 k2                                           (the caller's spectrum)
+//   pass 3  untangle in place: E = (Z[k] + conj Z[M-k]) / 2, O = (Z[k] - conj Z[M-k]) / 2i,
+//           X[k] = E + W^k O, X[M-k] = conj(E - W^k O), W = exp(-2 pi i / n)
+//
+// The in-CTA transform is an in-place radix-4 decimation in frequency (two fused radix-2 levels per shared-memory
+// round trip, a last radix-2 level when log2 R is odd); its bit-reversed order is undone when the tile is read
+// back out, so no separate re-ordering pass exists (PAPER.md:156-180 uses the same property).  All twiddles
+// come from fp64-evaluated tables: exp(-2 pi i j / R) per pass and a two-level table of exp(-2 pi i t / n).
+// HBM traffic: 3 x (8M read + 8M write) = 24 n bytes against the compulsory 8 n (4 n in, 4 n out).
+#pragma once
+#include "fdas_fft.cuh"
+#include <stdint.h>
+
+namespace fdas {
+
+struct R2CParams {
+    const float2 *in;     // pass 1: the time series as M complex; pass 2: work; pass 3: unused
+    float2 *out;          // pass 1: work; pass 2 / 3: the spectrum
+    const float2 *wR;     // exp(-2 pi i j / R), j < R (this pass's transform length)
+    const float2 *tlo;    // exp(-2 pi i t / n), t < 4096
+    const float2 *thi;    // exp(-2 pi i 4096 t / n), t < ceil(n / 4096)
+    long long M;          // n / 2
+    int M1, M2;           // M = M1 * M2
+    int log2R;            // log2 of this pass's transform length
+    int tile;             // transforms per CTA
+    float scale;
+};
+
+#ifdef __CUDACC__
+
+__device__ __forceinline__ float2 r2c_wn(const R2CParams &p, long long t)   // exp(-2 pi i t / n), 0 <= t < n
+{
+    return cmul(__ldg(p.thi + (t >> 12)), __ldg(p.tlo + (t & 4095)));
+}
+
+// In-place DIF of `tile` transforms of length R = 2^log2R held in buf[c * RS + i]; output bit-reversed.
+__device__ __forceinline__ void r2c_fft_tile(float2 *buf, int RS, int tile, int log2R, const float2 *__restrict__ wR)
+{
+    const int R = 1 << log2R;
+    int len = R;
+    for (; len >= 4; len >>= 2) {
+        const int q = len >> 2, wstep = R / len;
+        const int nb = tile * (R >> 2);
+        for (int e = threadIdx.x; e < nb; e += blockDim.x) {
+            const int c = e / (R >> 2), b = e - c * (R >> 2);
+            const int blk = b / q, j = b - blk * q;
+            float2 *a = buf + c * RS + blk * len + j;
+            const float2 a0 = a[0], a1 = a[q], a2 = a[2 * q], a3 = a[3 * q];
+            const float2 b0 = cadd(a0, a2), b1 = cadd(a1, a3);
+            const float2 b2 = cmul(csub(a0, a2), __ldg(wR + j * wstep));
+            const float2 b3 = cmul(csub(a1, a3), __ldg(wR + (j + q) * wstep));
+            const float2 w2 = __ldg(wR + 2 * j * wstep);
+            a[0] = cadd(b0, b1);
+            a[q] = cmul(csub(b0, b1), w2);
+            a[2 * q] = cadd(b2, b3);
+            a[3 * q] = cmul(csub(b2, b3), w2);
+        }
+        __syncthreads();
+    }
+    if (len == 2) {
+        const int nb = tile * (R >> 1);
+        for (int e = threadIdx.x; e < nb; e += blockDim.x) {
+            const int c = e / (R >> 1), b = e - c * (R >> 1);
+            float2 *a = buf + c * RS + 2 * b;
+            const float2 a0 = a[0], a1 = a[1];
+            a[0] = cadd(a0, a1);
+            a[1] = csub(a0, a1);
+        }
+        __syncthreads();
+    }
+}
+
+// pass 1: columns.  grid = M2 / tile
+__global__ void __launch_bounds__(256) r2c_pass1_kernel(const R2CParams p)
+{
+    extern __shared__ __align__(16) unsigned char r2c_smem[];
+    float2 *buf = reinterpret_cast<float2 *>(r2c_smem);
+    const int R = p.M1, RS = R + 1, tile = p.tile;
+    const long long j2_0 = (long long)blockIdx.x * tile;
+    for (int e = threadIdx.x; e < tile * R; e += blockDim.x) {
+        const int c = e % tile, j1 = e / tile;
+        buf[c * RS + j1] = __ldg(p.in + (long long)j1 * p.M2 + j2_0 + c);
+    }
+    __syncthreads();
+    r2c_fft_tile(buf, RS, tile, p.log2R, p.wR);
+    const int sh = 32 - p.log2R;
+    for (int e = threadIdx.x; e < tile * R; e += blockDim.x) {
+        const int c = e % tile, k1 = e / tile;
+        const float2 v = buf[c * RS + (int)(__brev((unsigned)k1) >> sh)];
+        const long long j2 = j2_0 + c;
+        p.out[(long long)k1 * p.M2 + j2] = cmul(v, r2c_wn(p, 2 * j2 * k1));   // exp(-2 pi i j2 k1 / M)
+    }
+}
+
+// pass 2: rows.  grid = M1 / tile
+__global__ void __launch_bounds__(256) r2c_pass2_kernel(const R2CParams p)
+{
+    extern __shared__ __align__(16) unsigned char r2c_smem[];
+    float2 *buf = reinterpret_cast<float2 *>(r2c_smem);
+    const int R = p.M2, RS = R + 1, tile = p.tile;
+    const long long k1_0 = (long long)blockIdx.x * tile;
+    for (int e = threadIdx.x; e < tile * R; e += blockDim.x) {
+        const int c = e / R, j2 = e - c * R;
+        buf[c * RS + j2] = __ldg(p.in + (k1_0 + c) * p.M2 + j2);
+    }
+    __syncthreads();
+    r2c_fft_tile(buf, RS, tile, p.log2R, p.wR);
+    const int sh = 32 - p.log2R;
+    for (int e = threadIdx.x; e < tile * R; e += blockDim.x) {
+        const int c = e % tile, k2 = e / tile;
+        p.out[k1_0 + c + (long long)p.M1 * k2] = buf[c * RS + (int)(__brev((unsigned)k2) >> sh)];
+    }
+}
+
+// pass 3: Z -> X in place, one thread per pair (k, M - k), k = 0 .. M/2
+__global__ void __launch_bounds__(256) r2c_untangle_kernel(const R2CParams p)
+{
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k > p.M / 2) return;
+    float2 *z = p.out;
+    if (k == 0) {
+        const float2 a = z[0];
+        z[0] = make_float2(p.scale * (a.x + a.y), 0.f);       // DC; the Nyquist bin a.x - a.y is dropped (R17)
+        return;
+    }
+    const float2 a = z[k], b = z[p.M - k];
+    const float2 e = make_float2(0.5f * (a.x + b.x), 0.5f * (a.y - b.y));     // (a + conj b) / 2
+    const float2 o = make_float2(0.5f * (a.y + b.y), -0.5f * (a.x - b.x));    // (a - conj b) / 2i
+    const float2 wo = cmul(o, r2c_wn(p, k));
+    z[k] = make_float2(p.scale * (e.x + wo.x), p.scale * (e.y + wo.y));
+    if (k != p.M - k) z[p.M - k] = make_float2(p.scale * (e.x - wo.x), -p.scale * (e.y - wo.y));
+}
+
+// exp(-2 pi i j step / len) for j < count, fp64-evaluated
+__global__ void r2c_table_kernel(float2 *tab, long long count, long long step, long long len)
+{
+    const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= count) return;
+    const long long t = (j * step) % len;
+    double s, c;
+    sincospi(-2.0 * (double)t / (double)len, &s, &c);
+    tab[j] = make_float2((float)c, (float)s);
+}
+
+#endif // __CUDACC__
+
+} // namespace fdas

@@ -16,6 +16,7 @@
 #include "fdas_kernel8k.cuh"
 #include "fdas_kernel2.cuh"
 #include "fdas_kernel3.cuh"
+#include "fdas_r2c.cuh"
 
 namespace fdas {
 
@@ -203,6 +204,30 @@ __global__ void fp32_peak_kernel(float *out, int iters, float a, float b)
     }
     const float s = v0 + v1 + v2 + v3 + v4 + v5 + v6 + v7;
     if (s == 12345.678f) out[0] = s;
+}
+
+// Harmonic summing of a stored plane + threshold (fdas_harmonic_sum_threshold, include/fdas.h; PAPER.md:73, :79,
+// :331; reading R18): thread <-> fundamental column c of row blockIdx.y, S = sum_h P[row(h z_k)][h c].
+__global__ void __launch_bounds__(256) harmonic_sum_kernel(const float *__restrict__ plane, long long ncols, int K,
+                                                           int nharm, int row_first, float threshold, Candidate *cands,
+                                                           long long capacity, unsigned long long *count)
+{
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long nc = (ncols - 1) / nharm + 1;
+    if (c >= nc) return;
+    const int k = row_first + blockIdx.y, center = (K - 1) / 2;
+    float s = 0.f;
+    for (int h = 1; h <= nharm; ++h) s += __ldg(plane + (size_t)(center + h * (k - center)) * ncols + h * c);
+    if (s > threshold) {
+        const unsigned long long slot = atomicAdd(count, 1ull);
+        if (slot < (unsigned long long)capacity) {
+            Candidate cd;
+            cd.col = c;
+            cd.row = k;
+            cd.power = s;
+            cands[slot] = cd;
+        }
+    }
 }
 
 } // namespace fdas

@@ -22,7 +22,8 @@ EXPORTS = ["fdas_plan_create", "fdas_make_templates", "fdas_execute", "fdas_exec
            "fdas_execute_threshold_host",
            "fdas_destroy",
            "fdas_plan_info", "fdas_get_taps", "fdas_get_template_spectrum", "fdas_measure_fp32_peak",
-           "fdas_launch_count", "fdas_status_string", "fdas_last_error"]
+           "fdas_launch_count", "fdas_status_string", "fdas_last_error",
+           "fdas_harmonic_sum_threshold", "fdas_r2c_plan_create", "fdas_r2c_execute", "fdas_r2c_destroy"]
 
 
 class FdasInfo(ctypes.Structure):
@@ -59,6 +60,10 @@ def _load() -> ctypes.CDLL:
     lib.fdas_execute_threshold.argtypes = [vp, vp, vp, ctypes.c_float, vp, i64, vp]
     lib.fdas_execute_threshold_host.argtypes = [vp, vp, vp, ctypes.c_float, vp, i64, vp]
     lib.fdas_destroy.argtypes = [vp]
+    lib.fdas_harmonic_sum_threshold.argtypes = [vp, vp, vp, i32, ctypes.c_float, vp, i64, vp]
+    lib.fdas_r2c_plan_create.argtypes = [ctypes.POINTER(vp), i64]
+    lib.fdas_r2c_execute.argtypes = [vp, vp, vp, vp, ctypes.c_float]
+    lib.fdas_r2c_destroy.argtypes = [vp]
     lib.fdas_plan_info.argtypes = [vp, ctypes.POINTER(FdasInfo)]
     lib.fdas_get_taps.argtypes = [vp, i32, vp, ctypes.POINTER(i32)]
     lib.fdas_get_template_spectrum.argtypes = [vp, i32, vp]
@@ -138,6 +143,32 @@ def fdas_execute_threshold_host(plan: int, stream, h_spectrum, threshold: float,
                                            int(capacity), _ptr(h_count)), "fdas_execute_threshold_host", plan)
 
 
+def fdas_harmonic_sum_threshold(plan: int, stream, d_plane, nharm: int, threshold: float, d_cands, capacity: int,
+                                d_count) -> None:
+    """Cells of the `nharm`-harmonic sum of a stored plane above `threshold` (candidate layout as above; row = bank
+    row of the fundamental, col = its column)."""
+    _check(lib.fdas_harmonic_sum_threshold(plan, _stream(stream), _ptr(d_plane), int(nharm), float(threshold),
+                                           _ptr(d_cands), int(capacity), _ptr(d_count)),
+           "fdas_harmonic_sum_threshold", plan)
+
+
+def fdas_r2c_plan_create(nsamples: int) -> int:
+    h = ctypes.c_void_p()
+    st = lib.fdas_r2c_plan_create(ctypes.byref(h), int(nsamples))
+    if st != FDAS_OK:
+        raise FdasError(st, "fdas_r2c_plan_create", lib.fdas_last_error(None).decode())
+    return h.value
+
+
+def fdas_r2c_execute(plan: int, stream, d_timeseries, d_spectrum, scale: float = 1.0) -> None:
+    _check(lib.fdas_r2c_execute(plan, _stream(stream), _ptr(d_timeseries), _ptr(d_spectrum), float(scale)),
+           "fdas_r2c_execute")
+
+
+def fdas_r2c_destroy(plan: int) -> None:
+    _check(lib.fdas_r2c_destroy(plan), "fdas_r2c_destroy")
+
+
 def fdas_destroy(plan: int) -> None:
     _check(lib.fdas_destroy(plan), "fdas_destroy")
 
@@ -203,12 +234,44 @@ class Plan:
     def execute_threshold_host(self, stream, h_spectrum, threshold, h_cands, capacity, h_count):
         fdas_execute_threshold_host(self.handle, stream, h_spectrum, threshold, h_cands, capacity, h_count)
 
+    def harmonic_sum_threshold(self, stream, d_plane, nharm, threshold, d_cands, capacity, d_count):
+        fdas_harmonic_sum_threshold(self.handle, stream, d_plane, nharm, threshold, d_cands, capacity, d_count)
+
     def execute_host(self, stream, h_spectrum, h_plane):
         fdas_execute_host(self.handle, stream, h_spectrum, h_plane)
 
     def close(self):
         if self.handle:
             fdas_destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class R2CPlan:
+    """RAII wrapper of the real-to-complex transform: R2CPlan(nsamples).execute(stream, d_series, d_spectrum, scale)."""
+
+    def __init__(self, nsamples):
+        self.handle = fdas_r2c_plan_create(nsamples)
+        self.nsamples = int(nsamples)
+        self.nbins = int(nsamples) // 2
+
+    def execute(self, stream, d_timeseries, d_spectrum, scale=1.0):
+        fdas_r2c_execute(self.handle, stream, d_timeseries, d_spectrum, scale)
+
+    def close(self):
+        if self.handle:
+            fdas_r2c_destroy(self.handle)
             self.handle = None
 
     def __enter__(self):

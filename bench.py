@@ -304,8 +304,10 @@ def run_table4():
     dev = torch.device("cuda", 0)
     stream = torch.cuda.Stream(device=dev)
     rows = []
+    peaks = load_peaks()
     for n, per_k in PAPER_TABLE4.items():
         N = n // 2
+        r2c_ms = time_r2c(torch, fdas, dev, stream, n, peaks, 10)["ms"]      # the long FFT the paper's times include
         spec = torch.from_numpy(synthetic.noise_only_c64(N, 4000 + n % 97).view(np.float32).reshape(N, 2)).to(dev)
         for K, counts in per_k.items():
             for ib in (0, 1):
@@ -328,10 +330,11 @@ def run_table4():
                             best = (ms, seglen)
                         del out
                 rows.append({"n_samples": n, "bins": N, "templates": K + 1, "interbin": ib, "seglen": best[1],
-                             "ms": round(best[0], 4),
+                             "ms": round(best[0], 4), "r2c_ms": round(r2c_ms, 4), "ms_incl_r2c": round(best[0] + r2c_ms, 4),
                              "paper_p100_ms_incl_r2c_fft": round(n * 64e-6 / counts[ib] * 1e3, 3)})
-    print(json.dumps({"sweep": "paper Table 4 shape (PAPER.md:319, :335-366); this library's time excludes the R2C FFT "
-                               "the paper's includes; other hardware: context, not a target", "rows": rows}))
+    print(json.dumps({"sweep": "paper Table 4 shape (PAPER.md:319, :335-366); ms = fdas_execute alone, ms_incl_r2c adds "
+                               "fdas_r2c_execute of the n-sample series, as the paper's times do; other hardware: context, "
+                               "not a target", "rows": rows}))
 
 
 KERNEL_OF_SEGLEN = {1024: "fdas_fused_kernel", 2048: "fdas_fused_kernel3", 4096: "fdas_fused_kernel2",
@@ -389,6 +392,66 @@ def time_config(torch, fdas, synthetic, dev, stream, w, steps, warmup, seed_off=
     del d_in, d_out
     torch.cuda.empty_cache()
     return ms, rec
+
+
+def time_r2c(torch, fdas, dev, stream, n, peaks, steps=20):
+    """fdas_r2c_execute on n real samples (the long FFT in front of the correlations):
+    three launches per call; HBM-bound, so its roofline is bytes: compulsory 4n in + 4n out."""
+    x = torch.randn(n, dtype=torch.float32, device=dev)
+    out = torch.empty((n // 2, 2), dtype=torch.float32, device=dev)
+    with fdas.R2CPlan(n) as plan:
+        with torch.cuda.stream(stream):
+            for _ in range(3):
+                plan.execute(stream, x, out, 1.0)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(steps):
+                plan.execute(stream, x, out, 1.0)
+            e1.record(stream)
+        stream.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    gbs = 8.0 * n / (ms * 1e-3) / 1e9
+    return {"nsamples": n, "ms": ms, "samples_per_s": n / (ms * 1e-3), "launches_per_call": 3,
+            "alg_bytes": 8 * n, "design_bytes": 24 * n, "achieved_gbs": gbs, "frac_hbm": gbs / peaks["hbm_gbs"],
+            "frac_hbm_of_design_traffic": 3.0 * gbs / peaks["hbm_gbs"],
+            "l2": "2^21 samples (8 MB in, 8 MB out, 8 MB work) stay in the 126 MB L2 between calls; 2^23 and 2^24 do not"
+                  if n <= (1 << 22) else "working set 3 x %d MB > 126 MB L2" % (4 * n >> 20)}
+
+
+def time_harmonics(torch, fdas, synthetic, dev, stream, w, peaks):
+    """fdas_harmonic_sum_threshold over a stored plane of config `w` for H = 2, 4, 8, 16."""
+    import numpy as np
+    N = w["nbins"]
+    with fdas.Plan(N, w["zmax"], w["dz"], w["seglen"], w["interbin"]) as plan:
+        plan.make_templates()
+        K, ncols = plan.info.ntemplates, plan.info.ncols
+        d_spec = torch.from_numpy(synthetic.noise_only_c64(N, 31).view(np.float32).reshape(N, 2)).to(dev)
+        d_plane = torch.empty((K, ncols), dtype=torch.float32, device=dev)
+        cap = 1 << 20
+        d_cands = torch.empty(cap * 16, dtype=torch.uint8, device=dev)
+        d_count = torch.zeros(1, dtype=torch.int64, device=dev)
+        out = {}
+        with torch.cuda.stream(stream):
+            plan.execute(stream, d_spec, d_plane)
+        for H in (2, 4, 8, 16):
+            thr = H + 6.0 * math.sqrt(H) + 6.0
+            with torch.cuda.stream(stream):
+                for _ in range(2):
+                    plan.harmonic_sum_threshold(stream, d_plane, H, thr, d_cands, cap, d_count)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                for _ in range(10):
+                    plan.harmonic_sum_threshold(stream, d_plane, H, thr, d_cands, cap, d_count)
+                e1.record(stream)
+            stream.synchronize()
+            rows = 2 * (((K - 1) // 2) // H) + 1
+            nc = (ncols - 1) // H + 1
+            ms = e0.elapsed_time(e1) / 10
+            out[str(H)] = {"ms": ms, "summed_cells": rows * nc, "cells_read": rows * nc * H,
+                           "read_gbs": 4.0 * rows * nc * H / (ms * 1e-3) / 1e9, "threshold": thr,
+                           "candidates": int(d_count.item())}
+    return {"workload": w["name"], "what": "S_H[z][r] = sum_h P[h z][h r] of the stored plane + threshold, one launch per H",
+            "harmonics": out}
 
 
 def self_launch(args):
@@ -613,6 +676,13 @@ def main():
                 "traffic": rc["traffic"], "traffic_source": rc["traffic_source"], "kernel": rc["kernel"],
                 "templates": wc["K"], "nbins": wc["nbins"], "seglen": wc["seglen"], "interbin": wc["interbin"],
                 "ctas_per_sm": rec["ctas_per_sm"], "regs": rec["regs"]}
+    extra = {}
+    if rank == 0 and world == 1 and not args.no_configs:
+        try:
+            extra["r2c"] = {str(n): time_r2c(torch, fdas, dev, stream, n, peaks) for n in (1 << 21, 1 << 23, 1 << 24)}
+            extra["harmonic_sum"] = time_harmonics(torch, fdas, synthetic, dev, stream, workload(2), peaks)
+        except Exception as exc:                      # the next-row extras must not cost the bench line
+            extra["extras_unavailable"] = f"{type(exc).__name__}: {exc}"[:200]
     dist.barrier()
 
     if rank == 0:
@@ -639,6 +709,7 @@ def main():
         }
         if others:
             out["configs"] = others
+        out.update(extra)
         out["threshold_search"] = {
             "what": "fdas_execute_threshold: same fused kernel, cells with P > threshold appended to a candidate "
                     "list instead of the plane store (paper's stated next step, PAPER.md:73, :331); per spectrum",

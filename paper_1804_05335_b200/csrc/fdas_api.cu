@@ -515,6 +515,8 @@ fdas_status fdas_get_template_spectrum(fdas_plan *p, int32_t k, float *host_re_i
 // ---------------------------------------------------------------- real-to-complex transform (fdas_r2c.cuh)
 } // extern "C"
 
+constexpr int R2C_THREADS = 512;
+
 struct fdas_r2c_plan {
     int64_t n, M;
     int device, M1, M2, log2M1, log2M2, tile1, tile2;
@@ -540,14 +542,14 @@ fdas_status fdas_r2c_plan_create(fdas_r2c_plan **out, int64_t nsamples)
     p->log2M2 = (p2 - 1) - p->log2M1;
     p->M1 = 1 << p->log2M1;
     p->M2 = 1 << p->log2M2;
-    auto tile_for = [](int R, int other) {          // transforms per CTA: <= 16384 points, <= 32, <= what exists
-        int t = 16384 / R;
-        if (t > 32) t = 32;
-        if (t > other) t = other;
-        return t;
+    auto ltile_for = [](int log2R, int log2other) {  // log2 of the transforms per CTA: <= 8192 points, <= 32, <= what exists
+        int t = 13 - log2R;
+        if (t > 5) t = 5;
+        if (t > log2other) t = log2other;
+        return t < 0 ? 0 : t;
     };
-    p->tile1 = tile_for(p->M1, p->M2);
-    p->tile2 = tile_for(p->M2, p->M1);
+    p->tile1 = ltile_for(p->log2M1, p->log2M2);
+    p->tile2 = ltile_for(p->log2M2, p->log2M1);
     g_create_err[0] = 0;
     const int64_t nhi = (nsamples + 4095) / 4096;
     cudaError_t e = cudaGetDevice(&p->device);
@@ -565,7 +567,7 @@ fdas_status fdas_r2c_plan_create(fdas_r2c_plan **out, int64_t nsamples)
         e = cudaDeviceSynchronize();
     }
     for (const void *k : {(const void *)r2c_pass1_kernel, (const void *)r2c_pass2_kernel})
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (16384 + 32) * 8);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (8192 + 32 + 4096) * 8);
     if (e != cudaSuccess) {
         snprintf(g_create_err, sizeof(g_create_err), "fdas_r2c_plan_create: %s", cudaGetErrorString(e));
         const bool nomem = e == cudaErrorMemoryAllocation;
@@ -596,13 +598,13 @@ fdas_status fdas_r2c_execute(fdas_r2c_plan *p, void *stream, const float *d_time
     q.wR = p->d_w1;
     q.log2R = p->log2M1;
     q.tile = p->tile1;
-    r2c_pass1_kernel<<<p->M2 / p->tile1, 256, (size_t)p->tile1 * (p->M1 + 1) * sizeof(float2), st>>>(q);
+    r2c_pass1_kernel<<<p->M2 >> p->tile1, R2C_THREADS, (((size_t)(p->M1 + 1) << p->tile1) + p->M1) * sizeof(float2), st>>>(q);
     q.in = p->d_work;
     q.out = (float2 *)d_spectrum;
     q.wR = p->d_w2;
     q.log2R = p->log2M2;
     q.tile = p->tile2;
-    r2c_pass2_kernel<<<p->M1 / p->tile2, 256, (size_t)p->tile2 * (p->M2 + 1) * sizeof(float2), st>>>(q);
+    r2c_pass2_kernel<<<p->M1 >> p->tile2, R2C_THREADS, (((size_t)(p->M2 + 1) << p->tile2) + p->M2) * sizeof(float2), st>>>(q);
     r2c_untangle_kernel<<<(unsigned)((p->M / 2 + 1 + 255) / 256), 256, 0, st>>>(q);
     g_launches += 3;
     if (cudaGetLastError() != cudaSuccess) return FDAS_ERR_CUDA;

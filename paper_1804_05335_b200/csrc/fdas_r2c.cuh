@@ -35,7 +35,7 @@ struct R2CParams {
     long long M;          // n / 2
     int M1, M2;           // M = M1 * M2
     int log2R;            // log2 of this pass's transform length
-    int tile;             // transforms per CTA
+    int tile;             // log2 of the transforms per CTA
     float scale;
 };
 
@@ -46,23 +46,24 @@ __device__ __forceinline__ float2 r2c_wn(const R2CParams &p, long long t)   // e
     return cmul(__ldg(p.thi + (t >> 12)), __ldg(p.tlo + (t & 4095)));
 }
 
-// In-place DIF of `tile` transforms of length R = 2^log2R held in buf[c * RS + i]; output bit-reversed.
-__device__ __forceinline__ void r2c_fft_tile(float2 *buf, int RS, int tile, int log2R, const float2 *__restrict__ wR)
+// In-place DIF of 2^ltile transforms of length R = 2^log2R held in buf[c * RS + i]; output bit-reversed.
+// sw: exp(-2 pi i j / R) in shared memory.  All index arithmetic is shifts and masks (R, tile are powers of two).
+__device__ __forceinline__ void r2c_fft_tile(float2 *buf, int RS, int ltile, int log2R, const float2 *sw)
 {
-    const int R = 1 << log2R;
-    int len = R;
-    for (; len >= 4; len >>= 2) {
-        const int q = len >> 2, wstep = R / len;
-        const int nb = tile * (R >> 2);
+    const int lq4 = log2R - 2;                            // log2 of the radix-4 butterflies per transform
+    int ll = log2R;                                       // log2 of the current block length
+    for (; ll >= 2; ll -= 2) {
+        const int lq = ll - 2, q = 1 << lq, ws = log2R - ll;
+        const int nb = 1 << (ltile + lq4);
         for (int e = threadIdx.x; e < nb; e += blockDim.x) {
-            const int c = e / (R >> 2), b = e - c * (R >> 2);
-            const int blk = b / q, j = b - blk * q;
-            float2 *a = buf + c * RS + blk * len + j;
+            const int c = e >> lq4, b = e & ((1 << lq4) - 1);
+            const int blk = b >> lq, j = b & (q - 1);
+            float2 *a = buf + c * RS + (blk << ll) + j;
             const float2 a0 = a[0], a1 = a[q], a2 = a[2 * q], a3 = a[3 * q];
             const float2 b0 = cadd(a0, a2), b1 = cadd(a1, a3);
-            const float2 b2 = cmul(csub(a0, a2), __ldg(wR + j * wstep));
-            const float2 b3 = cmul(csub(a1, a3), __ldg(wR + (j + q) * wstep));
-            const float2 w2 = __ldg(wR + 2 * j * wstep);
+            const float2 b2 = cmul(csub(a0, a2), sw[j << ws]);
+            const float2 b3 = cmul(csub(a1, a3), sw[(j + q) << ws]);
+            const float2 w2 = sw[(2 * j) << ws];
             a[0] = cadd(b0, b1);
             a[q] = cmul(csub(b0, b1), w2);
             a[2 * q] = cadd(b2, b3);
@@ -70,10 +71,10 @@ __device__ __forceinline__ void r2c_fft_tile(float2 *buf, int RS, int tile, int 
         }
         __syncthreads();
     }
-    if (len == 2) {
-        const int nb = tile * (R >> 1);
+    if (ll == 1) {
+        const int nb = 1 << (ltile + log2R - 1);
         for (int e = threadIdx.x; e < nb; e += blockDim.x) {
-            const int c = e / (R >> 1), b = e - c * (R >> 1);
+            const int c = e >> (log2R - 1), b = e & ((1 << (log2R - 1)) - 1);
             float2 *a = buf + c * RS + 2 * b;
             const float2 a0 = a[0], a1 = a[1];
             a[0] = cadd(a0, a1);
@@ -84,21 +85,23 @@ __device__ __forceinline__ void r2c_fft_tile(float2 *buf, int RS, int tile, int 
 }
 
 // pass 1: columns.  grid = M2 / tile
-__global__ void __launch_bounds__(256) r2c_pass1_kernel(const R2CParams p)
+__global__ void __launch_bounds__(1024) r2c_pass1_kernel(const R2CParams p)
 {
     extern __shared__ __align__(16) unsigned char r2c_smem[];
     float2 *buf = reinterpret_cast<float2 *>(r2c_smem);
-    const int R = p.M1, RS = R + 1, tile = p.tile;
-    const long long j2_0 = (long long)blockIdx.x * tile;
-    for (int e = threadIdx.x; e < tile * R; e += blockDim.x) {
-        const int c = e % tile, j1 = e / tile;
+    const int R = p.M1, RS = R + 1, lt = p.tile, tile = 1 << lt;
+    float2 *sw = buf + tile * RS;
+    const long long j2_0 = (long long)blockIdx.x << lt;
+    for (int e = threadIdx.x; e < R; e += blockDim.x) sw[e] = __ldg(p.wR + e);
+    for (int e = threadIdx.x; e < (R << lt); e += blockDim.x) {
+        const int c = e & (tile - 1), j1 = e >> lt;
         buf[c * RS + j1] = __ldg(p.in + (long long)j1 * p.M2 + j2_0 + c);
     }
     __syncthreads();
-    r2c_fft_tile(buf, RS, tile, p.log2R, p.wR);
+    r2c_fft_tile(buf, RS, lt, p.log2R, sw);
     const int sh = 32 - p.log2R;
-    for (int e = threadIdx.x; e < tile * R; e += blockDim.x) {
-        const int c = e % tile, k1 = e / tile;
+    for (int e = threadIdx.x; e < (R << lt); e += blockDim.x) {
+        const int c = e & (tile - 1), k1 = e >> lt;
         const float2 v = buf[c * RS + (int)(__brev((unsigned)k1) >> sh)];
         const long long j2 = j2_0 + c;
         p.out[(long long)k1 * p.M2 + j2] = cmul(v, r2c_wn(p, 2 * j2 * k1));   // exp(-2 pi i j2 k1 / M)
@@ -106,21 +109,23 @@ __global__ void __launch_bounds__(256) r2c_pass1_kernel(const R2CParams p)
 }
 
 // pass 2: rows.  grid = M1 / tile
-__global__ void __launch_bounds__(256) r2c_pass2_kernel(const R2CParams p)
+__global__ void __launch_bounds__(1024) r2c_pass2_kernel(const R2CParams p)
 {
     extern __shared__ __align__(16) unsigned char r2c_smem[];
     float2 *buf = reinterpret_cast<float2 *>(r2c_smem);
-    const int R = p.M2, RS = R + 1, tile = p.tile;
-    const long long k1_0 = (long long)blockIdx.x * tile;
-    for (int e = threadIdx.x; e < tile * R; e += blockDim.x) {
-        const int c = e / R, j2 = e - c * R;
+    const int R = p.M2, RS = R + 1, lt = p.tile, tile = 1 << lt;
+    float2 *sw = buf + tile * RS;
+    const long long k1_0 = (long long)blockIdx.x << lt;
+    for (int e = threadIdx.x; e < R; e += blockDim.x) sw[e] = __ldg(p.wR + e);
+    for (int e = threadIdx.x; e < (R << lt); e += blockDim.x) {
+        const int c = e >> p.log2R, j2 = e & (R - 1);
         buf[c * RS + j2] = __ldg(p.in + (k1_0 + c) * p.M2 + j2);
     }
     __syncthreads();
-    r2c_fft_tile(buf, RS, tile, p.log2R, p.wR);
+    r2c_fft_tile(buf, RS, lt, p.log2R, sw);
     const int sh = 32 - p.log2R;
-    for (int e = threadIdx.x; e < tile * R; e += blockDim.x) {
-        const int c = e % tile, k2 = e / tile;
+    for (int e = threadIdx.x; e < (R << lt); e += blockDim.x) {
+        const int c = e & (tile - 1), k2 = e >> lt;
         p.out[k1_0 + c + (long long)p.M1 * k2] = buf[c * RS + (int)(__brev((unsigned)k2) >> sh)];
     }
 }

@@ -185,13 +185,13 @@ typedef struct fdas_r2c_plan fdas_r2c_plan; /* opaque; created/destroyed by the 
  * correlations take (PAPER.md:79 Fig. 2, :105 "cuFFT R2C", :190, :219; eq. 5; reading R17):
  *     X[k] = scale * sum_j x[j] exp(-2 pi i j k / nsamples),  k = 0 .. nsamples/2 - 1
  * (DC kept, the Nyquist bin dropped).  nsamples must be a power of two, 2^10 <= nsamples <= 2^25
- * (FDAS_ERR_UNSUPPORTED otherwise).  Allocates a work array of nsamples/2 complex64 and the twiddle tables
+ * (FDAS_ERR_UNSUPPORTED otherwise).  Allocates two work arrays of nsamples/2 complex64 each and the twiddle tables
  * on the current device and fills the tables (synchronises once).
  */
 fdas_status fdas_r2c_plan_create(fdas_r2c_plan **out, int64_t nsamples);
 
 /*
- * Transform one series: three launches on `stream` (column transforms, row transforms, untangle), no host
+ * Transform one series: four launches on `stream` (three transform passes, untangle), no host
  * synchronisation, no allocation.
  *   d_timeseries : device, nsamples float32, 8-byte aligned; read only.
  *   d_spectrum   : device, nsamples/2 x {float re, float im}, 16-byte aligned; every bin is written.  It can be

@@ -519,8 +519,10 @@ constexpr int R2C_THREADS = 512;
 
 struct fdas_r2c_plan {
     int64_t n, M;
-    int device, M1, M2, log2M1, log2M2, tile1, tile2;
-    float2 *d_work, *d_w1, *d_w2, *d_tlo, *d_thi;
+    int device;
+    int lg[3];           // log2 of N1, N2, N3
+    int lt[3];           // log2 of the transforms per CTA in passes A, B, C
+    float2 *d_work[2], *d_w[3], *d_tlo, *d_thi;
 };
 
 extern "C" {
@@ -538,36 +540,41 @@ fdas_status fdas_r2c_plan_create(fdas_r2c_plan **out, int64_t nsamples)
     std::memset(p, 0, sizeof(*p));
     p->n = nsamples;
     p->M = nsamples / 2;
-    p->log2M1 = (p2 - 1) / 2;
-    p->log2M2 = (p2 - 1) - p->log2M1;
-    p->M1 = 1 << p->log2M1;
-    p->M2 = 1 << p->log2M2;
-    auto ltile_for = [](int log2R, int log2other) {  // log2 of the transforms per CTA: <= 8192 points, <= 32, <= what exists
-        int t = 13 - log2R;
-        if (t > 5) t = 5;
-        if (t > log2other) t = log2other;
-        return t < 0 ? 0 : t;
+    const int lm = p2 - 1;                               // M = N1 N2 N3, factors as equal as possible (<= 2^8)
+    p->lg[0] = lm / 3;
+    p->lg[1] = (lm - p->lg[0]) / 2;
+    p->lg[2] = lm - p->lg[0] - p->lg[1];
+    // transforms per CTA: 32 (one warp of columns), fewer where a dimension is shorter; <= 8192 points per CTA
+    auto ltile_for = [](int log2R, int log2avail) {
+        int t = 5;
+        if (t > log2avail) t = log2avail;
+        if (t > 13 - log2R) t = 13 - log2R;
+        return t;
     };
-    p->tile1 = ltile_for(p->log2M1, p->log2M2);
-    p->tile2 = ltile_for(p->log2M2, p->log2M1);
+    p->lt[0] = ltile_for(p->lg[0], p->lg[1] + p->lg[2]);
+    p->lt[1] = ltile_for(p->lg[1], p->lg[2]);
+    p->lt[2] = ltile_for(p->lg[2], p->lg[0]);
     g_create_err[0] = 0;
     const int64_t nhi = (nsamples + 4095) / 4096;
     cudaError_t e = cudaGetDevice(&p->device);
-    if (e == cudaSuccess) e = cudaMalloc(&p->d_work, (size_t)p->M * sizeof(float2));
-    if (e == cudaSuccess) e = cudaMalloc(&p->d_w1, (size_t)p->M1 * sizeof(float2));
-    if (e == cudaSuccess) e = cudaMalloc(&p->d_w2, (size_t)p->M2 * sizeof(float2));
+    for (int i = 0; i < 2; ++i)
+        if (e == cudaSuccess) e = cudaMalloc(&p->d_work[i], (size_t)p->M * sizeof(float2));
+    for (int i = 0; i < 3; ++i)
+        if (e == cudaSuccess) e = cudaMalloc(&p->d_w[i], (sizeof(float2)) << p->lg[i]);
     if (e == cudaSuccess) e = cudaMalloc(&p->d_tlo, 4096 * sizeof(float2));
     if (e == cudaSuccess) e = cudaMalloc(&p->d_thi, (size_t)nhi * sizeof(float2));
     if (e == cudaSuccess) {
-        r2c_table_kernel<<<(p->M1 + 127) / 128, 128>>>(p->d_w1, p->M1, 1, p->M1);
-        r2c_table_kernel<<<(p->M2 + 127) / 128, 128>>>(p->d_w2, p->M2, 1, p->M2);
+        for (int i = 0; i < 3; ++i) {
+            const long long R = 1ll << p->lg[i];
+            r2c_table_kernel<<<(unsigned)((R + 127) / 128), 128>>>(p->d_w[i], R, 1, R);
+        }
         r2c_table_kernel<<<32, 128>>>(p->d_tlo, 4096, 1, nsamples);
         r2c_table_kernel<<<(unsigned)((nhi + 127) / 128), 128>>>(p->d_thi, nhi, 4096, nsamples);
-        g_launches += 4;
+        g_launches += 5;
         e = cudaDeviceSynchronize();
     }
-    for (const void *k : {(const void *)r2c_pass1_kernel, (const void *)r2c_pass2_kernel})
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (8192 + 32 + 4096) * 8);
+    for (const void *k : {(const void *)r2c_cols_kernel, (const void *)r2c_rows_kernel})
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (8192 + 32 + 256) * 8);
     if (e != cudaSuccess) {
         snprintf(g_create_err, sizeof(g_create_err), "fdas_r2c_plan_create: %s", cudaGetErrorString(e));
         const bool nomem = e == cudaErrorMemoryAllocation;
@@ -586,27 +593,45 @@ fdas_status fdas_r2c_execute(fdas_r2c_plan *p, void *stream, const float *d_time
     if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device) return FDAS_ERR_INVALID_ARG;
     if (((uintptr_t)d_timeseries & 7) || ((uintptr_t)d_spectrum & 15)) return FDAS_ERR_ALIGNMENT;
     cudaStream_t st = (cudaStream_t)stream;
+    const long long N1 = 1ll << p->lg[0], N2 = 1ll << p->lg[1], N3 = 1ll << p->lg[2];
+    auto smem = [](int lg, int lt) { return ((((size_t)1 << lg) + 1) << lt) * sizeof(float2) + (sizeof(float2) << lg); };
     R2CParams q;
     q.tlo = p->d_tlo;
     q.thi = p->d_thi;
     q.M = p->M;
-    q.M1 = p->M1;
-    q.M2 = p->M2;
+    q.N1 = (int)N1;
+    q.N2 = (int)N2;
     q.scale = scale;
+    // pass A: length N1 over j1, columns j' = j2 N3 + j3
     q.in = (const float2 *)d_timeseries;
-    q.out = p->d_work;
-    q.wR = p->d_w1;
-    q.log2R = p->log2M1;
-    q.tile = p->tile1;
-    r2c_pass1_kernel<<<p->M2 >> p->tile1, R2C_THREADS, (((size_t)(p->M1 + 1) << p->tile1) + p->M1) * sizeof(float2), st>>>(q);
-    q.in = p->d_work;
+    q.out = p->d_work[0];
+    q.wR = p->d_w[0];
+    q.log2R = p->lg[0];
+    q.ltile = p->lt[0];
+    q.inner = N2 * N3;
+    q.slab = p->M;
+    q.tmul = 2;
+    r2c_cols_kernel<<<dim3((unsigned)((N2 * N3) >> p->lt[0]), 1), R2C_THREADS, smem(p->lg[0], p->lt[0]), st>>>(q);
+    // pass B: per k1, length N2 over j2, columns j3
+    q.in = p->d_work[0];
+    q.out = p->d_work[1];
+    q.wR = p->d_w[1];
+    q.log2R = p->lg[1];
+    q.ltile = p->lt[1];
+    q.inner = N3;
+    q.slab = N2 * N3;
+    q.tmul = 2 * N1;
+    r2c_cols_kernel<<<dim3((unsigned)(N3 >> p->lt[1]), (unsigned)N1), R2C_THREADS, smem(p->lg[1], p->lt[1]), st>>>(q);
+    // pass C: length N3 over j3, transposed store
+    q.in = p->d_work[1];
     q.out = (float2 *)d_spectrum;
-    q.wR = p->d_w2;
-    q.log2R = p->log2M2;
-    q.tile = p->tile2;
-    r2c_pass2_kernel<<<p->M1 >> p->tile2, R2C_THREADS, (((size_t)(p->M2 + 1) << p->tile2) + p->M2) * sizeof(float2), st>>>(q);
+    q.wR = p->d_w[2];
+    q.log2R = p->lg[2];
+    q.ltile = p->lt[2];
+    q.inner = N3;
+    r2c_rows_kernel<<<dim3((unsigned)(N1 >> p->lt[2]), (unsigned)N2), R2C_THREADS, smem(p->lg[2], p->lt[2]), st>>>(q);
     r2c_untangle_kernel<<<(unsigned)((p->M / 2 + 1 + 255) / 256), 256, 0, st>>>(q);
-    g_launches += 3;
+    g_launches += 4;
     if (cudaGetLastError() != cudaSuccess) return FDAS_ERR_CUDA;
     return FDAS_OK;
 }
@@ -614,9 +639,8 @@ fdas_status fdas_r2c_execute(fdas_r2c_plan *p, void *stream, const float *d_time
 fdas_status fdas_r2c_destroy(fdas_r2c_plan *p)
 {
     if (!p) return FDAS_OK;
-    cudaFree(p->d_work);
-    cudaFree(p->d_w1);
-    cudaFree(p->d_w2);
+    for (int i = 0; i < 2; ++i) cudaFree(p->d_work[i]);
+    for (int i = 0; i < 3; ++i) cudaFree(p->d_w[i]);
     cudaFree(p->d_tlo);
     cudaFree(p->d_thi);
     cudaGetLastError();

@@ -5,21 +5,26 @@
 //
 //     X[k] = scale * sum_{j=0}^{n-1} x[j] exp(-2 pi i j k / n),   k = 0 .. n/2 - 1     (reading R17: DC kept,
 //                                                                                       Nyquist bin dropped)
-// n = 2^p real samples.  The series is read as M = n/2 complex numbers z[j] = x[2j] + i x[2j+1]; Z = DFT_M(z) by the
-// four-step decomposition M = M1 * M2 (j = j1 M2 + j2, k = k1 + M1 k2), two passes through HBM:
+// n = 2^p real samples.  The series is read as M = n/2 complex numbers z[j] = x[2j] + i x[2j+1]; Z = DFT_M(z) by a
+// three-factor decomposition M = N1 N2 N3 (j = j1 N2 N3 + j2 N3 + j3, k = k1 + N1 k2 + N1 N2 k3; every factor
+// <= 256), i.e. the four-step scheme applied twice, three passes through memory plus the untangle:
 //
-//   pass 1  one CTA per tile of adjacent columns j2: length-M1 transforms over j1 in shared memory,
-//           times exp(-2 pi i j2 k1 / M), stored at [k1][j2]                      (plan-owned work array)
-//   pass 2  one CTA per tile of adjacent rows k1: length-M2 transforms over j2 in shared memory, stored
-//           transposed at k = k1 + M1 k2                                           (the caller's spectrum)
-//   pass 3  untangle in place: E = (Z[k] + conj Z[M-k]) / 2, O = (Z[k] - conj Z[M-k]) / 2i,
+//   pass A  transforms of length N1 over j1 (stride N2 N3), times exp(-2 pi i j' k1 / M), j' = j2 N3 + j3  -> [k1][j']
+//   pass B  per k1: transforms of length N2 over j2 (stride N3), times exp(-2 pi i j3 k2 / (N2 N3))         -> [k1][k2][j3]
+//   pass C  transforms of length N3 over j3 (contiguous), stored transposed at k = k1 + N1 k2 + N1 N2 k3    -> spectrum
+//   pass D  untangle in place: E = (Z[k] + conj Z[M-k]) / 2, O = (Z[k] - conj Z[M-k]) / 2i,
 //           X[k] = E + W^k O, X[M-k] = conj(E - W^k O), W = exp(-2 pi i / n)
 //
-// The in-CTA transform is an in-place radix-4 decimation in frequency (two fused radix-2 levels per shared-memory
-// round trip, a last radix-2 level when log2 R is odd); its bit-reversed order is undone when the tile is read
-// back out, so no separate re-ordering pass exists (PAPER.md:156-180 uses the same property).  All twiddles
-// come from fp64-evaluated tables: exp(-2 pi i j / R) per pass and a two-level table of exp(-2 pi i t / n).
-// HBM traffic: 3 x (8M read + 8M write) = 24 n bytes against the compulsory 8 n (4 n in, 4 n out).
+// A CTA holds 2^ltile transforms side by side in shared memory (rows padded to R + 1 elements).  In passes A and
+// B the side-by-side transforms are ADJACENT COLUMNS (the innermost, contiguous index), in pass C adjacent k1, so
+// every global access of every pass is a run of 2^ltile * 8 contiguous bytes (256 B at ltile = 5); inside the CTA
+// lane <-> transform, so butterflies, twiddle reads (one address per warp) and the bit-reversed read-out are free
+// of bank conflicts.  The in-CTA transform is an in-place radix-4 decimation in frequency (two fused radix-2
+// levels per shared-memory round trip, a last radix-2 level when log2 R is odd); its bit-reversed order is
+// undone when the tile is read back out, so no separate re-ordering pass exists (PAPER.md:156-180 uses the same
+// property).  All twiddles come from fp64-evaluated tables: exp(-2 pi i j / R) per pass and a two-level table of
+// exp(-2 pi i t / n).  Traffic: 4 x (8M read + 8M write) = 32 n bytes against the compulsory 8 n (4 n in, 4 n
+// out); up to n = 2^23 the 12 n-byte working set stays in the 126 MB L2 between passes.
 #pragma once
 #include "fdas_fft.cuh"
 #include <stdint.h>
@@ -27,15 +32,18 @@
 namespace fdas {
 
 struct R2CParams {
-    const float2 *in;     // pass 1: the time series as M complex; pass 2: work; pass 3: unused
-    float2 *out;          // pass 1: work; pass 2 / 3: the spectrum
+    const float2 *in;     // this pass's input
+    float2 *out;          // this pass's output
     const float2 *wR;     // exp(-2 pi i j / R), j < R (this pass's transform length)
     const float2 *tlo;    // exp(-2 pi i t / n), t < 4096
     const float2 *thi;    // exp(-2 pi i 4096 t / n), t < ceil(n / 4096)
     long long M;          // n / 2
-    int M1, M2;           // M = M1 * M2
-    int log2R;            // log2 of this pass's transform length
-    int tile;             // log2 of the transforms per CTA
+    long long inner;      // passes A / B: columns per slab (A: N2 N3, B: N3); pass C: N3
+    long long slab;       // passes A / B: elements per slab (A: M, B: N2 N3)
+    long long tmul;       // passes A / B: twiddle exp(-2 pi i tmul col k / n)  (A: 2, B: 2 N1)
+    int N1, N2;           // pass C: output index k1 + N1 k2 + N1 N2 k3
+    int log2R;            // log2 of this pass's transform length R
+    int ltile;            // log2 of the transforms per CTA
     float scale;
 };
 
@@ -50,13 +58,13 @@ __device__ __forceinline__ float2 r2c_wn(const R2CParams &p, long long t)   // e
 // sw: exp(-2 pi i j / R) in shared memory.  All index arithmetic is shifts and masks (R, tile are powers of two).
 __device__ __forceinline__ void r2c_fft_tile(float2 *buf, int RS, int ltile, int log2R, const float2 *sw)
 {
-    const int lq4 = log2R - 2;                            // log2 of the radix-4 butterflies per transform
+    const int tmask = (1 << ltile) - 1;
     int ll = log2R;                                       // log2 of the current block length
     for (; ll >= 2; ll -= 2) {
         const int lq = ll - 2, q = 1 << lq, ws = log2R - ll;
-        const int nb = 1 << (ltile + lq4);
+        const int nb = 1 << (ltile + log2R - 2);
         for (int e = threadIdx.x; e < nb; e += blockDim.x) {
-            const int c = e >> lq4, b = e & ((1 << lq4) - 1);
+            const int c = e & tmask, b = e >> ltile;      // lane <-> transform: conflict-free, twiddles broadcast
             const int blk = b >> lq, j = b & (q - 1);
             float2 *a = buf + c * RS + (blk << ll) + j;
             const float2 a0 = a[0], a1 = a[q], a2 = a[2 * q], a3 = a[3 * q];
@@ -74,7 +82,7 @@ __device__ __forceinline__ void r2c_fft_tile(float2 *buf, int RS, int ltile, int
     if (ll == 1) {
         const int nb = 1 << (ltile + log2R - 1);
         for (int e = threadIdx.x; e < nb; e += blockDim.x) {
-            const int c = e >> (log2R - 1), b = e & ((1 << (log2R - 1)) - 1);
+            const int c = e & tmask, b = e >> ltile;
             float2 *a = buf + c * RS + 2 * b;
             const float2 a0 = a[0], a1 = a[1];
             a[0] = cadd(a0, a1);
@@ -84,53 +92,55 @@ __device__ __forceinline__ void r2c_fft_tile(float2 *buf, int RS, int ltile, int
     }
 }
 
-// pass 1: columns.  grid = M2 / tile
-__global__ void __launch_bounds__(1024) r2c_pass1_kernel(const R2CParams p)
+// passes A and B: transforms over a strided index for 2^ltile adjacent columns.  grid = (inner >> ltile, slabs)
+__global__ void __launch_bounds__(512) r2c_cols_kernel(const R2CParams p)
 {
     extern __shared__ __align__(16) unsigned char r2c_smem[];
     float2 *buf = reinterpret_cast<float2 *>(r2c_smem);
-    const int R = p.M1, RS = R + 1, lt = p.tile, tile = 1 << lt;
+    const int R = 1 << p.log2R, RS = R + 1, lt = p.ltile, tile = 1 << lt;
     float2 *sw = buf + tile * RS;
-    const long long j2_0 = (long long)blockIdx.x << lt;
+    const long long col0 = (long long)blockIdx.x << lt;
+    const float2 *in = p.in + (long long)blockIdx.y * p.slab;
+    float2 *out = p.out + (long long)blockIdx.y * p.slab;
     for (int e = threadIdx.x; e < R; e += blockDim.x) sw[e] = __ldg(p.wR + e);
     for (int e = threadIdx.x; e < (R << lt); e += blockDim.x) {
-        const int c = e & (tile - 1), j1 = e >> lt;
-        buf[c * RS + j1] = __ldg(p.in + (long long)j1 * p.M2 + j2_0 + c);
+        const int c = e & (tile - 1), j = e >> lt;
+        buf[c * RS + j] = __ldg(in + (long long)j * p.inner + col0 + c);
     }
     __syncthreads();
     r2c_fft_tile(buf, RS, lt, p.log2R, sw);
     const int sh = 32 - p.log2R;
     for (int e = threadIdx.x; e < (R << lt); e += blockDim.x) {
-        const int c = e & (tile - 1), k1 = e >> lt;
-        const float2 v = buf[c * RS + (int)(__brev((unsigned)k1) >> sh)];
-        const long long j2 = j2_0 + c;
-        p.out[(long long)k1 * p.M2 + j2] = cmul(v, r2c_wn(p, 2 * j2 * k1));   // exp(-2 pi i j2 k1 / M)
+        const int c = e & (tile - 1), k = e >> lt;
+        const float2 v = buf[c * RS + (int)(__brev((unsigned)k) >> sh)];
+        out[(long long)k * p.inner + col0 + c] = cmul(v, r2c_wn(p, p.tmul * (col0 + c) * k));
     }
 }
 
-// pass 2: rows.  grid = M1 / tile
-__global__ void __launch_bounds__(1024) r2c_pass2_kernel(const R2CParams p)
+// pass C: transforms over the contiguous index j3 of the rows (k1, k2), 2^ltile adjacent k1 per CTA.
+// grid = (N1 >> ltile, N2)
+__global__ void __launch_bounds__(512) r2c_rows_kernel(const R2CParams p)
 {
     extern __shared__ __align__(16) unsigned char r2c_smem[];
     float2 *buf = reinterpret_cast<float2 *>(r2c_smem);
-    const int R = p.M2, RS = R + 1, lt = p.tile, tile = 1 << lt;
+    const int R = 1 << p.log2R, RS = R + 1, lt = p.ltile, tile = 1 << lt;
     float2 *sw = buf + tile * RS;
-    const long long k1_0 = (long long)blockIdx.x << lt;
+    const long long k1_0 = (long long)blockIdx.x << lt, k2 = blockIdx.y;
     for (int e = threadIdx.x; e < R; e += blockDim.x) sw[e] = __ldg(p.wR + e);
     for (int e = threadIdx.x; e < (R << lt); e += blockDim.x) {
-        const int c = e >> p.log2R, j2 = e & (R - 1);
-        buf[c * RS + j2] = __ldg(p.in + (k1_0 + c) * p.M2 + j2);
+        const int c = e >> p.log2R, j3 = e & (R - 1);
+        buf[c * RS + j3] = __ldg(p.in + ((k1_0 + c) * p.N2 + k2) * R + j3);
     }
     __syncthreads();
     r2c_fft_tile(buf, RS, lt, p.log2R, sw);
     const int sh = 32 - p.log2R;
     for (int e = threadIdx.x; e < (R << lt); e += blockDim.x) {
-        const int c = e & (tile - 1), k2 = e >> lt;
-        p.out[k1_0 + c + (long long)p.M1 * k2] = buf[c * RS + (int)(__brev((unsigned)k2) >> sh)];
+        const int c = e & (tile - 1), k3 = e >> lt;
+        p.out[k1_0 + c + (long long)p.N1 * (k2 + (long long)p.N2 * k3)] = buf[c * RS + (int)(__brev((unsigned)k3) >> sh)];
     }
 }
 
-// pass 3: Z -> X in place, one thread per pair (k, M - k), k = 0 .. M/2
+// pass D: Z -> X in place, one thread per pair (k, M - k), k = 0 .. M/2
 __global__ void __launch_bounds__(256) r2c_untangle_kernel(const R2CParams p)
 {
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;

@@ -437,6 +437,37 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
                  "@!p bra WAIT_%=;\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
 
+// ------------------------------------------------------------------ bulk copy of a segment (TMA engine, 1-D)
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}"
+                 ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// global -> this CTA's shared memory, completion counted in bytes on `bar` (cp.async.bulk: SASS UBLKCP)
+__device__ __forceinline__ void bulk_load(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+// F1 from a segment already in shared memory: DFT16 over n1, twiddle, store E1 (as fwd_f1 of fdas_kernel.cuh)
+// (STRIDE / OFF as fwd_f1: the transform's input n is element STRIDE n + OFF of the segment)
+template <int L, int STRIDE = 1, int OFF = 0>
+__device__ __forceinline__ void fwd_f1_smem(const float2 *seg, const float2 *__restrict__ wtab, const ThreadMap<L> &tm,
+                                            float2 *e1)
+{
+    using G = Geo<L>;
+    const int t1 = tm.tid;
+    float2 a[16];
+#pragma unroll
+    for (int n1 = 0; n1 < 16; ++n1) a[n1] = seg[STRIDE * (n1 * G::Q + t1) + OFF];
+    dft<-1, 16>(a);
+#pragma unroll
+    for (int k1 = 0; k1 < 16; ++k1) {
+        const float2 v = (k1 == 0) ? a[0] : cmul(a[k1], wtab[(k1 * t1) & (L - 1)]);
+        e1[k1 * G::S1 + t1] = v;
+    }
+}
+
 // Interbin cells whose neighbour y[n+1] lives in another warp (lane 31 of every warp) are finished
 // one unit late from the two small "own" / "edge" mailboxes written during Q1.
 template <int L>

@@ -38,7 +38,7 @@ struct Geo2 : Geo<L> {
     static_assert(G::KM == G::R3 && (G::R3 == 8 || G::R3 == 16), "shuffle exchange: L = 2048 or 4096");
     static constexpr int smem_bytes(bool interbin)
     {
-        return 32 /* full[2], empty[2] */ + 2 * G::E1_ELEMS * 16 + (interbin ? G::EDGE_ELEMS * 16 : 0);
+        return 32 /* full[2], empty[2] */ + 2 * G::E1_ELEMS * 16 + (interbin ? G::EDGE_ELEMS * 16 : 0) + 16 /* segment barrier */;
     }
 };
 
@@ -199,6 +199,8 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
     uint64_t *empty = full + 2;                                              // empty[0], empty[1]
     float2 *e1base = reinterpret_cast<float2 *>(smem_raw + 32);              // two (re, im) buffers
     float4 *edges = reinterpret_cast<float4 *>(e1base + 4 * G::E1_ELEMS);    // interbin only
+    // bulk segment load: transaction barrier in the last 16 bytes of the allocation
+    uint64_t *segbar = reinterpret_cast<uint64_t *>(smem_raw + 32 + 2 * G::E1_ELEMS * 16 + (INTERBIN ? G::EDGE_ELEMS * 16 : 0));
     const ThreadMap<L> tm(threadIdx.x);
     const int tid = tm.tid;
 
@@ -207,6 +209,8 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
         mbar_init(&full[1], G::T);
         mbar_init(&empty[0], G::T);
         mbar_init(&empty[1], G::T);
+        mbar_init(segbar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");   // visible to the async proxy
     }
     __syncthreads();
 
@@ -321,6 +325,7 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
     // Per unit u: [forward transform at a segment start] produce(u); then consume u-1 (same
     // segment) and, at the end of the segment or of this CTA's range, u itself.  A whole unit of
     // other work lies between a warp's arrive on full[u & 1] and its wait on it.
+    unsigned nbulk = 0;                                        // bulk segment loads so far (phase of `segbar`)
     for (int u = 0; u < n; ++u) {
         const bool first = (u == 0) || (pair == 0);
         if (first) {
@@ -329,8 +334,20 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel2(const Kern
                 if (pend[0].on) flush_edges<L, MODE>(prm, tm, edges, pend[0]);
                 if (pend[1].on) flush_edges<L, MODE>(prm, tm, edges, pend[1]);
             }
-            float2 *scr = e1base + 2 * G::E1_ELEMS;            // second buffer: F2 -> F3 scratch
-            fwd_f1<L>(prm.spectrum, prm.nbins, seg * prm.useful - prm.overlap, prm.wtab, tm, e1base);
+            float2 *scr = e1base + 2 * G::E1_ELEMS;            // second buffer: segment landing zone, then F2 -> F3 scratch
+            const long long seg_start = seg * prm.useful - prm.overlap;
+            if (seg_start >= 0 && seg_start + L <= prm.nbins) {    // a2: one bulk copy (TMA engine) of the segment
+                if (tid == 0) {
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    mbar_expect_tx(segbar, L * (uint32_t)sizeof(float2));
+                    bulk_load(scr, prm.spectrum + seg_start, L * (uint32_t)sizeof(float2), segbar);
+                }
+                mbar_wait(segbar, nbulk & 1);
+                ++nbulk;
+                fwd_f1_smem<L>(scr, prm.wtab, tm, e1base);
+            } else {                                               // first / last segments: zero extension (R7)
+                fwd_f1<L>(prm.spectrum, prm.nbins, seg_start, prm.wtab, tm, e1base);
+            }
             __syncthreads();
             fwd_f2<L>(prm.wtab, tm, e1base, scr);
             __syncwarp();

@@ -273,11 +273,14 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel3(const Kern
     const int tid = tm.tid;
     const int g = tm.n3;                                                     // index inside the exchange group
 
+    uint64_t *segbar = reinterpret_cast<uint64_t *>(smem_raw + 40);          // bulk segment load: transaction barrier
     if (tid == 0) {
         mbar_init(&full[0], G::T);
         mbar_init(&full[1], G::T);
         mbar_init(&empty[0], G::T);
         mbar_init(&empty[1], G::T);
+        mbar_init(segbar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");   // visible to the async proxy
     }
     constexpr bool PARK = MINB >= 3;                                         // X^ / twiddles in tensor memory
     if (PARK && tm.warp == 0) tmem_alloc<G3::TM_COLS>(tslot);
@@ -490,6 +493,7 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel3(const Kern
             }
         };
 
+        unsigned nbulk = 0;                                        // bulk segment loads so far (phase of `segbar`)
         // Per unit u: [forward transform at a segment start] produce(u); then consume u-1 (same
         // segment) and, at the end of the segment or of this CTA's range, u itself.
         for (int u = 0; u < n; ++u) {
@@ -498,8 +502,22 @@ __global__ void __launch_bounds__(Geo<L>::T, MINB) fdas_fused_kernel3(const Kern
                 __syncthreads();                                   // every earlier unit is consumed
                 flush(0);
                 flush(1);
-                float2 *scr = e1base + 2 * G::E1_ELEMS;            // second buffer: F2 -> F3 scratch
-                fwd_f1<L>(prm.spectrum, prm.nbins, seg * prm.useful - prm.overlap, prm.wtab, tm, e1base);
+                float2 *scr = e1base + 2 * G::E1_ELEMS;            // second buffer: segment landing zone, then F2 -> F3 scratch
+                const long long seg_start = seg * prm.useful - prm.overlap;
+                if (seg_start >= 0 && seg_start + L <= prm.nbins) {
+                    // a2 (the segment goes to shared memory once): one bulk copy of the L bins by the
+                    // TMA engine, completion counted in bytes on `segbar`; every thread waits, then reads its 16 bins
+                    if (tid == 0) {
+                        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic accesses of `scr`
+                        mbar_expect_tx(segbar, L * (uint32_t)sizeof(float2));
+                        bulk_load(scr, prm.spectrum + seg_start, L * (uint32_t)sizeof(float2), segbar);
+                    }
+                    mbar_wait(segbar, nbulk & 1);
+                    ++nbulk;
+                    fwd_f1_smem<L>(scr, prm.wtab, tm, e1base);
+                } else {                                           // first / last segments: zero extension (reading R7)
+                    fwd_f1<L>(prm.spectrum, prm.nbins, seg_start, prm.wtab, tm, e1base);
+                }
                 __syncthreads();
                 fwd_f2<L>(prm.wtab, tm, e1base, scr);
                 __syncwarp();

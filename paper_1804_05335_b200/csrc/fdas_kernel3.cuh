@@ -108,6 +108,14 @@ __device__ __forceinline__ void tmem_ld(uint32_t taddr, uint32_t (&v)[32])
                  "tcgen05.wait::ld.sync.aligned;"
                  : FDAS_L8(v, 0), FDAS_L8(v, 8), FDAS_L8(v, 16), FDAS_L8(v, 24) : "r"(taddr));
 }
+// two 16-word loads, one wait
+__device__ __forceinline__ void tmem_ld2(uint32_t ta, uint32_t (&a)[16], uint32_t tb, uint32_t (&b)[16])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%32];\n\t"
+                 "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%33];\n\t"
+                 "tcgen05.wait::ld.sync.aligned;"
+                 : FDAS_L8(a, 0), FDAS_L8(a, 8), FDAS_L8(b, 0), FDAS_L8(b, 8) : "r"(ta), "r"(tb));
+}
 __device__ __forceinline__ void tmem_st(uint32_t taddr, const uint32_t (&v)[32])
 {
     asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "

@@ -7,7 +7,7 @@
 //   forward, once per segment (decimation in time over the INPUT parity):
 //       Ee = DFT_4096(x[2n]),  Oo = DFT_4096(x[2n+1]),   W = exp(-2 pi i / 8192)
 //       X^[k] = Ee[k] + W^k Oo[k],   X^[k+4096] = Ee[k] - W^k Oo[k],   k < 4096
-//     both halves go to a thread-private 64 KB shared-memory array (slot order of Geo<4096>).
+//     both halves go to the thread's 64 words of tensor memory (slot order of Geo<4096>).
 //   inverse, per (slot, parity pi) sub-unit (decimation in frequency over the OUTPUT parity):
 //       y[2n'+pi] = IDFT_4096( ( (X^H)[k] + (-1)^pi (X^H)[k+4096] ) conj(W)^(pi k) )[n']
 //     the Q3 input stage forms the two products (for H and conj H), their sum or
@@ -25,18 +25,19 @@
 // interbinned 8192 slot therefore costs two plain ones (the paper's own interbinning cost was x1.1-1.6
 // on top of the transform; the shuffle epilogue of the smaller segment lengths is x1.4).
 //
-// With X^ in shared memory only ONE E1 buffer fits: the split-phase `full` barrier is paired
-// with an `empty` barrier (arrive after Q1's loads, wait before Q2's stores).
+// X^ (both halves, 64 words per thread, lane-private and read once per sub-unit) lives in TENSOR MEMORY
+// (tcgen05.st once per segment, two tcgen05.ld.x16 per eight slots), which frees the 64 KB of shared memory it
+// took in round 1: E1 is double-buffered behind one split-phase `full` barrier per buffer, as in fdas_kernel.cuh.
 #pragma once
-#include "fdas_kernel.cuh"
+#include "fdas_kernel3.cuh"
 
 namespace fdas {
 
 struct Geo8k {
     using G = Geo<4096>;
     static constexpr int L = 8192;
-    static constexpr int XS_ELEMS = 2 * G::PTS * G::T; // float2: X^lo[16][T], X^hi[16][T]
-    static constexpr int smem_bytes() { return 32 + (G::E2_ELEMS + G::E1_ELEMS) * 16 + XS_ELEMS * 8; }
+    static constexpr int TM_COLS = 128;                // tensor memory: X^lo, X^hi (32 words each) per thread, two warp sets
+    static constexpr int smem_bytes() { return 32 + (G::E2_ELEMS + 2 * G::E1_ELEMS) * 16; }   // E2, two E1 buffers
 };
 
 #ifdef __CUDACC__
@@ -47,7 +48,7 @@ __device__ __forceinline__ constexpr float c32im(int i) { return sinw(i); }
 
 // Q3 of one parity: products, sum / twiddled difference, inverse DFT16 over k3, twiddle, store E2.
 template <int PARITY, int HALF = 0>
-__device__ __forceinline__ void inv_q3_8k(const float2 *xs_lo, const float2 *xs_hi, const float4 (&hlo)[8],
+__device__ __forceinline__ void inv_q3_8k(uint32_t tmw, const float4 (&hlo)[8],
                                           const float4 (&hhi)[8], float2 wb, const InvTwiddles<4096> &tw,
                                           const ThreadMap<4096> &tm, const XBuf &e2,
                                           const float2 *__restrict__ wtab2 = nullptr)
@@ -55,8 +56,13 @@ __device__ __forceinline__ void inv_q3_8k(const float2 *xs_lo, const float2 *xs_
     using G = Geo<4096>;
     cpk a[16];
 #pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        float2 xl = xs_lo[i * G::T + tm.tid], xh = xs_hi[i * G::T + tm.tid];
+    for (int c = 0; c < 2; ++c) {
+    uint32_t wl[16], wh[16];                           // X^lo / X^hi of slots 8c .. 8c+7 from tensor memory
+    tmem_ld2(tmw + 16 * c, wl, tmw + 32 + 16 * c, wh);
+#pragma unroll
+    for (int ii = 0; ii < 8; ++ii) {
+        const int i = 8 * c + ii;
+        float2 xl = w2f(wl, ii), xh = w2f(wh, ii);
         if constexpr (HALF) {
             // (pi/4)(1 -+ e) with e = exp(+2 pi i k / 8192), k = k1 + 16 k2 + 256 i (the slot of xl; xh is k + 4096)
             constexpr float S = 0.78539816339744830961566084581988f;
@@ -82,6 +88,7 @@ __device__ __forceinline__ void inv_q3_8k(const float2 *xs_lo, const float2 *xs_
         }
         a[i] = v;
     }
+    }
     if constexpr (PARITY) {
         // conj(W)^(256 i) = exp(+2 pi i i / 32): compile-time constants
 #pragma unroll
@@ -95,18 +102,41 @@ __device__ __forceinline__ void inv_q3_8k(const float2 *xs_lo, const float2 *xs_
     }
 }
 
+// Plain plane, one parity sub-unit: rows N1 .. N1+3 of both transforms, eight 4-byte streaming stores at immediate
+// offsets from the two row bases, each row under its own mask bit (the valid rows differ from lane to lane here: the
+// overlap in units of n' is a multiple of 16, not of 32).  Row step = 2 Q cells (the other parity sits in between).
+template <int N1>
+__device__ __forceinline__ void store_rows_8k(const cpk (&y)[16], float *bp, float *bq, unsigned vm)
+{
+    constexpr int RB = 2 * Geo<4096>::Q * 4;     // bytes between n1 rows
+    float2 pw[4];
+#pragma unroll
+    for (int r = 0; r < 4; ++r) pw[r] = power2(y[N1 + r]);
+    asm volatile("{\n\t.reg .pred p0, p1, p2, p3;\n\t.reg .b32 t;\n\t"
+                 "and.b32 t, %10, %15;\n\tsetp.ne.u32 p0, t, 0;\n\t"
+                 "and.b32 t, %10, %16;\n\tsetp.ne.u32 p1, t, 0;\n\t"
+                 "and.b32 t, %10, %17;\n\tsetp.ne.u32 p2, t, 0;\n\t"
+                 "and.b32 t, %10, %18;\n\tsetp.ne.u32 p3, t, 0;\n\t"
+                 "@p0 st.global.cs.f32 [%0+%11], %2;\n\t@p0 st.global.cs.f32 [%1+%11], %3;\n\t"
+                 "@p1 st.global.cs.f32 [%0+%12], %4;\n\t@p1 st.global.cs.f32 [%1+%12], %5;\n\t"
+                 "@p2 st.global.cs.f32 [%0+%13], %6;\n\t@p2 st.global.cs.f32 [%1+%13], %7;\n\t"
+                 "@p3 st.global.cs.f32 [%0+%14], %8;\n\t@p3 st.global.cs.f32 [%1+%14], %9;\n\t}"
+                 ::"l"(bp), "l"(bq), "f"(pw[0].x), "f"(pw[0].y), "f"(pw[1].x), "f"(pw[1].y), "f"(pw[2].x), "f"(pw[2].y),
+                   "f"(pw[3].x), "f"(pw[3].y), "r"(vm), "n"(N1 * RB), "n"((N1 + 1) * RB), "n"((N1 + 2) * RB),
+                   "n"((N1 + 3) * RB), "n"(1u << N1), "n"(2u << N1), "n"(4u << N1), "n"(8u << N1)
+                 : "memory");
+}
+
 template <int MINB, int MODE = 0, bool INTERBIN = false>
 __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelParams prm)
 {
     using G = Geo<4096>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    uint64_t *mbar = reinterpret_cast<uint64_t *>(smem_raw);                 // [0] full, [1] empty
+    uint64_t *mbar = reinterpret_cast<uint64_t *>(smem_raw);                 // full[0], full[1] (one per E1 buffer)
     float2 *sm = reinterpret_cast<float2 *>(smem_raw + 32);
     const XBuf e2{sm, sm + G::E2_ELEMS};
     float2 *e1base = sm + 2 * G::E2_ELEMS;
-    const XBuf e1{e1base, e1base + G::E1_ELEMS};
-    float2 *xs_lo = e1base + 2 * G::E1_ELEMS;
-    float2 *xs_hi = xs_lo + G::PTS * G::T;
+    uint32_t *tslot = reinterpret_cast<uint32_t *>(smem_raw + 16);
     const ThreadMap<4096> tm(threadIdx.x);
     const int tid = tm.tid;
 
@@ -114,7 +144,13 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
         mbar_init(&mbar[0], G::T);
         mbar_init(&mbar[1], G::T);
     }
+    // X^ (both halves, 64 words per thread) lives in tensor memory: lane-private, read once per sub-unit
+    if (tm.warp == 0) tmem_alloc<Geo8k::TM_COLS>(tslot);
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tm_base = *tslot;
+    const uint32_t tmw = tm_base + ((uint32_t)(32 * (tm.warp & 3)) << 16) + (uint32_t)(tm.warp >> 2) * 64u;
 
     InvTwiddles<4096> tw;
     load_inv_twiddles<4096>(prm.wtab, tm, tw);
@@ -128,7 +164,10 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
     const long long units = prm.nseg * prm.npairs;
     const long long u0 = units * blockIdx.x / gridDim.x;
     const int n = (int)(units * (blockIdx.x + 1) / gridDim.x - u0);
-    if (n <= 0) return;
+    if (n <= 0) {
+        if (tm.warp == 0) tmem_dealloc<Geo8k::TM_COLS>(tm_base);   // the whole CTA is idle
+        return;
+    }
     long long seg = u0 / prm.npairs;
     int pair = (int)(u0 - seg * prm.npairs);
 
@@ -160,7 +199,7 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
     // sub-units of a slot: s = par + 2 half (half = 1: the interbin difference transform)
     constexpr int SUBS = INTERBIN ? 4 : 2;
     constexpr int CS = INTERBIN ? 2 : 1;              // plane columns per bin
-#define FDAS_Q3_SUB(PAR, HALF) inv_q3_8k<PAR, HALF>(xs_lo, xs_hi, hlo, hhi, wb, tw, tm, e2, prm.wtab2)
+#define FDAS_Q3_SUB(PAR, HALF) inv_q3_8k<PAR, HALF>(tmw, hlo, hhi, wb, tw, tm, e2, prm.wtab2)
     // parked (p, q) powers of sub-units 0..2, see the epilogue.  (The same parking for the plain plane -- parity 0
     // waits, parity 1 stores float2 pairs -- measured 4.35 ms against 3.98 ms for the stride-2 stores: not used.)
     float2 held[INTERBIN && MODE == 0 ? 48 : 1];
@@ -168,6 +207,7 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
     const int nsub = SUBS * n;
     for (int c = 0; c < nsub; ++c) {
         const int sub = c % SUBS;
+        const XBuf e1{e1base + (c & 1) * 2 * G::E1_ELEMS, e1base + (c & 1) * 2 * G::E1_ELEMS + G::E1_ELEMS};
         const int par = sub & 1, half = sub >> 1;
         if (!have_q3) {
             // first sub-unit of a segment for this CTA (always parity 0): forward transform
@@ -186,13 +226,21 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
             __syncwarp();
             fwd_f3<4096>(tm, e2.re, xo);
             __syncthreads();                                   // E1 / E2 are rewritten below
+            {
+                uint32_t wl[32], wh[32];
 #pragma unroll
-            for (int i = 0; i < 16; ++i) {
-                const float2 t = cmul(xo[i], prm.wtab2[tm.k1 + 16 * tm.k2m + 256 * i]);
-                xs_lo[i * G::T + tid] = cadd(xe[i], t);        // thread-private slots
-                xs_hi[i * G::T + tid] = csub(xe[i], t);
+                for (int i = 0; i < 16; ++i) {
+                    const float2 t = cmul(xo[i], prm.wtab2[tm.k1 + 16 * tm.k2m + 256 * i]);
+                    const float2 lo = cadd(xe[i], t), hi = csub(xe[i], t);
+                    wl[2 * i] = __float_as_uint(lo.x);
+                    wl[2 * i + 1] = __float_as_uint(lo.y);
+                    wh[2 * i] = __float_as_uint(hi.x);
+                    wh[2 * i + 1] = __float_as_uint(hi.y);
+                }
+                tmem_st(tmw, wl);
+                tmem_st(tmw + 32, wh);
             }
-            inv_q3_8k<0>(xs_lo, xs_hi, hlo, hhi, wb, tw, tm, e2);
+            inv_q3_8k<0>(tmw, hlo, hhi, wb, tw, tm, e2);
             __syncwarp();
         }
         // Q2: load E2, inverse DFT16 over k2, twiddle; E1 must be free before the stores
@@ -203,11 +251,12 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
             dft<+1, 16>(a);
 #pragma unroll
             for (int n2 = 0; n2 < 16; ++n2) a[n2] = cmul(a[n2], tw.tw2[n2]);
-            if (c > 0) mbar_wait(&mbar[1], (c - 1) & 1);       // every warp has loaded Q1(c-1)
+            // E1[c & 1]: every warp finished loading sub-unit c-2 from it before it arrived for c-1, and this
+            // warp has waited for c-1's arrivals -- no `empty` barrier with two buffers
 #pragma unroll
             for (int n2 = 0; n2 < 16; ++n2) e1.put(tm.e1_q2 + n2 * G::R3, a[n2]);
         }
-        mbar_arrive(&mbar[0]);
+        mbar_arrive(&mbar[c & 1]);
         __syncwarp();
 
         // Q3 of the next sub-unit of the same segment
@@ -224,7 +273,7 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
             }
             if (sub + 2 == SUBS) fetch_h();                    // next slot's H, one sub-unit ahead
         }
-        mbar_wait(&mbar[0], c & 1);
+        mbar_wait(&mbar[c & 1], (c >> 1) & 1);
 
         const int row_p = pair;
         const int row_q = prm.ntemplates - 1 - pair;
@@ -232,7 +281,6 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
         cpk y[16];
 #pragma unroll
         for (int k1 = 0; k1 < 16; ++k1) y[k1] = e1.get(k1 * G::S1 + tid);
-        mbar_arrive(&mbar[1]);                                 // E1 may be overwritten
         dft<+1, 16>(y);
         unsigned vm = vmask;
         if (col0 + prm.overlap + prm.useful > prm.nbins) {
@@ -279,7 +327,14 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
             float *bp = prm.plane + (size_t)row_p * prm.ncols + (CS * (col0 + 2 * tid + par) + half);
             float *bq = prm.plane + (size_t)row_q * prm.ncols + (CS * (col0 + 2 * tid + par) + half);
             const unsigned qon = (MODE != 0 && row_q == row_p) ? 0u : ~0u;   // MODE 1: z = 0 cell reported once
-            emit_unit<4096, false, MODE, 2 * CS>(prm, y, bp, bq, vm, vm & qon);
+            if constexpr (MODE == 0 && !INTERBIN) {
+                store_rows_8k<0>(y, bp, bq, vm);
+                store_rows_8k<4>(y, bp, bq, vm);
+                store_rows_8k<8>(y, bp, bq, vm);
+                store_rows_8k<12>(y, bp, bq, vm);
+            } else {
+                emit_unit<4096, false, MODE, 2 * CS>(prm, y, bp, bq, vm, vm & qon);
+            }
         }
         __syncwarp();
         if (sub == SUBS - 1 && ++pair == prm.npairs) {
@@ -287,6 +342,9 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
             ++seg;
         }
     }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (tm.warp == 0) tmem_dealloc<Geo8k::TM_COLS>(tm_base);
 }
 
 #undef FDAS_Q3_SUB

@@ -78,8 +78,7 @@ typedef struct fdas_info {
  * each template of half-width ceil(|z|/2)+16 bins (R4), segment FFT length `seglen`
  * ("blocks of length L"); `interbin` = 0: N columns; 1: 2N columns, half-bin cells
  * by interbinning (eq. 4), any seglen; 2: 2N columns, half-bin cells by two-bin
- * Fourier interpolation (a second template bank, twice the transforms;
- * seglen <= 4096, FDAS_ERR_UNSUPPORTED at 8192).
+ * Fourier interpolation (a second template bank, twice the transforms), any seglen.
  * Allocates the plan-owned device memory (taps, template spectra, twiddle table).
  * *out is set to NULL on failure.
  */

@@ -106,7 +106,7 @@ kernel_fn select_kernel(int L, int ib, int mode = 0)
     case 2048: return pick_kernel3<2048, K3_CTAS_PER_SM_2048>(ib, mode);
     case 4096: return pick_kernel2<4096, 1>(ib, mode);
     case 8192:                                                            // 2 x 4096 (fdas_kernel8k.cuh)
-        if (ib == 2) return nullptr;
+        if (ib == 2) return mode ? (kernel_fn)fdas_fused_kernel_8k<1, 1, false, 2> : (kernel_fn)fdas_fused_kernel_8k<1, 0, false, 2>;
         if (ib) return mode ? (kernel_fn)fdas_fused_kernel_8k<1, 1, true> : (kernel_fn)fdas_fused_kernel_8k<1, 0, true>;
         return mode ? (kernel_fn)fdas_fused_kernel_8k<1, 1> : (kernel_fn)fdas_fused_kernel_8k<1>;
     default: return nullptr;
@@ -301,7 +301,11 @@ fdas_status fdas_make_templates(fdas_plan *p, void *stream)
                 make_spectra_kernel<4096><<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps + (size_t)b * n, I.npairs, I.halfwidth,
                                                             I.zmax, I.dz, I.ntemplates, p->nbanks, b);
             break;
-        case 8192: make_spectra_kernel_8k<<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps, I.npairs, I.halfwidth, I.zmax, I.dz, I.ntemplates); break;
+        case 8192:
+            for (int b = 0; b < p->nbanks; ++b)
+                make_spectra_kernel_8k<<<gb, 128, 0, st>>>(p->d_hperm, p->d_taps + (size_t)b * n, I.npairs, I.halfwidth, I.zmax,
+                                                           I.dz, I.ntemplates, p->nbanks, b);
+            break;
         default: return FDAS_ERR_UNSUPPORTED;
         }
         g_launches += 3;

@@ -127,7 +127,10 @@ __device__ __forceinline__ void store_rows_8k(const cpk (&y)[16], float *bp, flo
                  : "memory");
 }
 
-template <int MINB, int MODE = 0, bool INTERBIN = false>
+// BANKS = 2 (two-bin Fourier interpolation, reading R16; plain sub-units only): prm.npairs counts
+// template SLOTS, slot = 2 * pair + bank, as in fdas_kernel.cuh: bank 0 fills the even plane columns, bank 1 (the
+// templates at half-integer offsets) the odd ones, and bank 1's q transform is the +|z| row shifted by one bin.
+template <int MINB, int MODE = 0, bool INTERBIN = false, int BANKS = 1>
 __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelParams prm)
 {
     using G = Geo<4096>;
@@ -194,6 +197,15 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
     for (int n1 = 0; n1 < 16; ++n1) {
         const int nn = n1 * G::Q + tid;
         if (nn >= ov2 && nn < ov2 + us2) vmask |= 1u << n1;
+    }
+
+    unsigned vmask_m1 = 0;                       // BANKS = 2, bank 1, q row, parity 0: bin 2n' - 1
+    if constexpr (BANKS == 2) {
+#pragma unroll
+        for (int n1 = 0; n1 < 16; ++n1) {
+            const int nn = n1 * G::Q + tid - 1;
+            if (nn >= ov2 && nn < ov2 + us2) vmask_m1 |= 1u << n1;
+        }
     }
 
     // sub-units of a slot: s = par + 2 half (half = 1: the interbin difference transform)
@@ -275,8 +287,9 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
         }
         mbar_wait(&mbar[c & 1], (c >> 1) & 1);
 
-        const int row_p = pair;
-        const int row_q = prm.ntemplates - 1 - pair;
+        const int bank = BANKS == 2 ? (pair & 1) : 0;
+        const int row_p = BANKS == 2 ? (pair >> 1) : pair;
+        const int row_q = prm.ntemplates - 1 - row_p;
         const long long col0 = seg * prm.useful - prm.overlap;
         cpk y[16];
 #pragma unroll
@@ -322,6 +335,18 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
                     st_stream2_if(bq + 4 * n1 * G::Q + 2, c2.y, c3.y, alq ? 0u : pb);
                 }
             }
+        } else if constexpr (BANKS == 2) {
+            // bin n = 2n' + par -> column 2 n + bank in row p; bank 1's q output n is the half-bin cell of bin n - 1
+            float *bp = prm.plane + (size_t)row_p * prm.ncols + (2 * (col0 + 2 * tid + par) + bank);
+            float *bq = prm.plane + (size_t)row_q * prm.ncols + (2 * (col0 + 2 * tid + par - bank) + bank);
+            unsigned vmq = (bank && par == 0) ? vmask_m1 : vmask;
+            if (col0 + prm.overlap + prm.useful >= prm.nbins) {
+#pragma unroll 1
+                for (int n1 = 0; n1 < 16; ++n1)
+                    if (col0 + 2 * (n1 * G::Q + tid) + par - bank >= prm.nbins) vmq &= ~(1u << n1);
+            }
+            if (row_q == row_p) vmq = 0;                       // z = 0 slot: its q row is the p row again
+            emit_unit<4096, false, MODE, 4>(prm, y, bp, bq, vm, vmq);
         } else {
             // bin n = 2n' + par -> plane column CS * (col0 + n) + half
             float *bp = prm.plane + (size_t)row_p * prm.ncols + (CS * (col0 + 2 * tid + par) + half);

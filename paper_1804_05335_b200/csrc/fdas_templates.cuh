@@ -162,7 +162,7 @@ __global__ void make_spectra_kernel(float2 *hperm, const double2 *taps, int npai
 // seglen 8192: hperm[pair][half][i/2][tid] with half 0 = H[k], half 1 = H[k + 4096], k < 4096 in
 // the slot order of Geo<4096> (fdas_kernel8k.cuh).
 __global__ void make_spectra_kernel_8k(float2 *hperm, const double2 *taps, int npairs, int m,
-                                       double zmax, double dz, int K)
+                                       double zmax, double dz, int K, int nbanks, int bank)
 {
     using G = Geo<4096>;
     constexpr int L = 8192;
@@ -186,7 +186,7 @@ __global__ void make_spectra_kernel_8k(float2 *hperm, const double2 *taps, int n
     int tid, i;
     freq_to_reg<4096>(f & 4095, tid, i);
     const int half = f >> 12;
-    const size_t off = ((((size_t)pair * 2 + half) * (G::PTS / 2) + (i >> 1)) * G::T + tid) * 2 + (i & 1);
+    const size_t off = (((((size_t)pair * nbanks + bank) * 2 + half) * (G::PTS / 2) + (i >> 1)) * G::T + tid) * 2 + (i & 1);
     hperm[off] = make_float2((float)(sr / L), (float)(si / L));
 }
 

@@ -49,7 +49,6 @@ def test_argument_errors_without_device(fd):
     assert lib.fdas_plan_create(ctypes.byref(h), 1024, 20.0, 0.0, 1024, 0) == 1
     assert lib.fdas_plan_create(ctypes.byref(h), 1024, 5.0, 2.0, 1024, 0) == 1       # zmax/dz not integer
     assert lib.fdas_plan_create(ctypes.byref(h), 1024, 20.0, 2.0, 1024, 3) == 1
-    assert lib.fdas_plan_create(ctypes.byref(h), 1 << 20, 200.0, 2.0, 8192, 2) == 2   # two-bin interpolation at 8192
     assert lib.fdas_plan_create(ctypes.byref(h), 1024, 20.0, 2.0, 1000, 0) == 2      # seglen
     assert lib.fdas_plan_create(ctypes.byref(h), 1024, 2000.0, 2.0, 1024, 0) == 2    # overlap >= seglen/2
     assert lib.fdas_plan_create(ctypes.byref(h), 1 << 20, 8100.0, 2.0, 8192, 1) == 2  # overlap >= seglen/2

@@ -27,6 +27,7 @@ sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
     (1 << 19, 200.0, 8192, 0),
     (1 << 19, 200.0, 8192, 1),
     (100003, 84.0, 8192, 1),
+    (1 << 18, 84.0, 8192, 2),
     (200_003, 20.0, 1024, 2),
     (300_001, 84.0, 2048, 2),
     (1 << 19, 84.0, 4096, 2),

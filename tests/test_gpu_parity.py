@@ -201,7 +201,8 @@ def test_seglen_8192_interbin(torch, fd, orc, syn, nbins, zmax):
 
 
 @pytest.mark.parametrize("nbins,zmax,seglen", [(1 << 15, 20.0, 1024), (50021, 84.0, 2048), (1 << 16, 84.0, 4096),
-                                               (3, 20.0, 1024), (1921, 84.0, 2048)])
+                                               (3, 20.0, 1024), (1921, 84.0, 2048), (1 << 16, 84.0, 8192),
+                                               (40003, 200.0, 8192), (7, 40.0, 8192)])
 def test_two_bin_fourier_interpolation(torch, fd, orc, syn, nbins, zmax, seglen):
     """interbin = 2 (reading R16): even columns = the plain plane, odd columns = the correlation
     with the templates at half-integer offsets (second template bank); against the oracle's zero-interleaved
@@ -360,7 +361,7 @@ def test_deterministic_and_linear(torch, fd, syn):
 
 
 @pytest.mark.parametrize("seglen,interbin", [(1024, 0), (1024, 1), (1024, 2), (2048, 0), (2048, 1), (2048, 2),
-                                             (4096, 0), (4096, 1), (4096, 2), (8192, 0), (8192, 1)])
+                                             (4096, 0), (4096, 1), (4096, 2), (8192, 0), (8192, 1), (8192, 2)])
 def test_bitwise_repeatable_all_kernels(torch, fd, syn, seglen, interbin):
     # compute-sanitizer is closed on this pool; a race in the shared-memory exchange pipeline
     # (split-phase mbarriers, per-warp regions, mailbox, tensor-memory parking) would show up as run-to-run

@@ -57,6 +57,7 @@ def check_against_oracle(orc, spec, zmax, dz, interbin, thr, rec):
     (1 << 17, 84.0, 4096, 1, 10.0),
     (1 << 17, 200.0, 8192, 0, 11.0),
     (1 << 16, 84.0, 8192, 1, 10.0),
+    (1 << 16, 84.0, 8192, 2, 10.0),
     (1 << 16, 84.0, 2048, 2, 10.0),
     (40009, 84.0, 4096, 2, 10.0),
 ])

@@ -337,7 +337,7 @@ def run_table4():
                                "not a target", "rows": rows}))
 
 
-KERNEL_OF_SEGLEN = {1024: "fdas_fused_kernel", 2048: "fdas_fused_kernel3", 4096: "fdas_fused_kernel2",
+KERNEL_OF_SEGLEN = {1024: "fdas_fused_kernel", 2048: "fdas_fused_kernel3", 4096: "fdas_fused_kernel2 (interbinned: fdas_fused_kernel3)",
                     8192: "fdas_fused_kernel_8k"}
 
 

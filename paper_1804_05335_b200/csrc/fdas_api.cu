@@ -86,7 +86,8 @@ kernel_fn pick_kernel2(int ib, int mode)
     return ib ? (kernel_fn)fdas_fused_kernel2<L, true, MINB> : (kernel_fn)fdas_fused_kernel2<L, false, MINB>;
 }
 
-// L = 2048: third-generation kernel (X^ and twiddles in tensor memory, three CTAs per SM, fdas_kernel3.cuh).
+// L = 2048: third-generation kernel (X^ and twiddles in tensor memory, three CTAs per SM, fdas_kernel3.cuh);
+// L = 4096 interbinned: the same kernel with X^ and twiddles in registers (one CTA per SM).
 template <int L, int MINB>
 kernel_fn pick_kernel3(int ib, int mode)
 {
@@ -104,7 +105,8 @@ kernel_fn select_kernel(int L, int ib, int mode = 0)
     switch (L) {
     case 1024: return pick_kernel<1024, 4>(ib, mode);
     case 2048: return pick_kernel3<2048, K3_CTAS_PER_SM_2048>(ib, mode);
-    case 4096: return pick_kernel2<4096, 1>(ib, mode);
+    case 4096:                                                            // measured per half-bin mode
+        return ib == 1 ? pick_kernel3<4096, 1>(ib, mode) : pick_kernel2<4096, 1>(ib, mode);
     case 8192:                                                            // 2 x 4096 (fdas_kernel8k.cuh)
         if (ib == 2) return mode ? (kernel_fn)fdas_fused_kernel_8k<1, 1, false, 2> : (kernel_fn)fdas_fused_kernel_8k<1, 0, false, 2>;
         if (ib) return mode ? (kernel_fn)fdas_fused_kernel_8k<1, 1, true> : (kernel_fn)fdas_fused_kernel_8k<1, 0, true>;
@@ -118,7 +120,7 @@ int smem_bytes_for(int L, bool ib)
     switch (L) {
     case 1024: return Geo<1024>::smem_bytes(ib);
     case 2048: return Geo3<2048>::smem_bytes(ib);
-    case 4096: return Geo2<4096>::smem_bytes(ib);
+    case 4096: return ib ? Geo3<4096>::smem_bytes(true) : Geo2<4096>::smem_bytes(false);
     case 8192: return Geo8k::smem_bytes();
     default: return 0;
     }

@@ -439,3 +439,29 @@ def test_fp32_peak_probe(torch, fd):
     tf = fd.fdas_measure_fp32_peak(None, 2000)
     assert 20.0 < tf < 90.0, tf
     assert fd.fdas_launch_count() > 0
+
+
+def test_two_plans_on_two_streams_share_the_gpu(torch, fd, orc, syn):
+    """Two plans of the tensor-memory kernels (seglen 2048: three CTAs per SM, 128 columns each; seglen 8192: 128
+    columns) enqueued on two streams at once: tensor-memory allocation and the persistent grids must coexist, and
+    both planes must still match the oracle."""
+    n = 1 << 18
+    spec_a = syn.make_spectrum(n, 501, [(0.3 * n, 10.0, 20.0)])
+    spec_b = syn.make_spectrum(n, 502, [(0.6 * n, -30.0, 25.0)])
+    with fd.Plan(n, 84.0, 2.0, 2048, 1) as pa, fd.Plan(n, 84.0, 2.0, 8192, 0) as pb:
+        pa.make_templates()
+        pb.make_templates()
+        torch.cuda.synchronize()
+        sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+        da = torch.from_numpy(spec_a.view(np.float32).reshape(n, 2)).cuda()
+        db = torch.from_numpy(spec_b.view(np.float32).reshape(n, 2)).cuda()
+        oa = torch.full((85, 2 * n), float("nan"), dtype=torch.float32, device="cuda")
+        ob = torch.full((85, n), float("nan"), dtype=torch.float32, device="cuda")
+        torch.cuda.synchronize()
+        for _ in range(4):                                  # interleaved launches, no host sync in between
+            pa.execute(sa, da, oa)
+            pb.execute(sb, db, ob)
+        sa.synchronize()
+        sb.synchronize()
+        check_rows(orc, spec_a, oa.cpu().numpy(), 84.0, 2.0, 1, rows=[0, 30, 47, 84])
+        check_rows(orc, spec_b, ob.cpu().numpy(), 84.0, 2.0, 0, rows=[0, 27, 42, 84])

@@ -1,4 +1,5 @@
-// Fused FDAS kernel, third generation (L = 2048, 4096): three CTAs per SM.
+// Fused FDAS kernel, third generation.  L = 2048 (BASELINE configs 2 and 5): X^ and twiddles in tensor memory,
+// three CTAs per SM.  L = 4096 interbinned (config 3): the same kernel with those values in registers, one CTA per SM.
 //
 // What round 1 measured (profiles/r1e_*): two warps per SM sub-partition at 237-255
 // registers, FMA pipe 47-59 % busy, the SM's load/store data pipe 69-72 % busy, and the issue slot idle more
@@ -7,7 +8,7 @@
 // read-only for a whole segment (X^) or for the whole launch (the inverse twiddles).
 //
 // This kernel keeps the second generation's structure (fdas_kernel2.cuh: Q3 -> Q2 transpose by warp
-// shuffles, produce / consume pipeline over a double-buffered E1) and changes three things:
+// shuffles, produce / consume pipeline over a double-buffered E1) and changes four things:
 //
 //   1. X^ and the inverse twiddles live in TENSOR MEMORY (256 KB per SM, lane-private in the 32x32b shape
 //      like a register file; tcgen05.st once per segment / launch, tcgen05.ld 16-32 words at a time just
@@ -22,7 +23,12 @@
 //      sign on the odd branch: +40 packed instructions per unit in fdas_kernel2.cuh).  The phase
 //      e^{2 pi i g n/8} is folded into the Q2 -> Q1 twiddles.
 //   3. Plane stores take their n1 offset as an immediate of the store instruction (one base address per
-//      row instead of a 64-bit add per cell).
+//      row instead of a 64-bit add per cell); interbinned rows go out four at a time under one predicate.
+//   4. The segment is fetched by ONE bulk copy of the TMA engine (cp.async.bulk + mbarrier transaction count)
+//      into the free E1 buffer (the segment goes to shared memory once); the first and last
+//      segments of a spectrum, which need the zero extension, keep the predicated loads.
+//
+// Measured effect of each change: DESIGN.md sections 4.2c and 6.
 //
 // Index maps (as fdas_kernel.cuh): n = n1 Q + n2 R3 + n3, k = k1 + 16 k2 + 256 k3; a warp owns C values
 // of k1, lane = k1l + C g, g < G = R3.  Q3: thread (k1, g) holds k2 = NB3 g + j, all k3.  Q2: thread

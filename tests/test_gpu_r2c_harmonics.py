@@ -74,9 +74,9 @@ def test_r2c_whole_spectrum_against_direct_sums(torch, fd, orc, n):
     assert got[0].imag == 0.0                                  # DC is real; the Nyquist bin is dropped (R17)
 
 
-@pytest.mark.parametrize("n", [1 << 17, 1 << 20, 1 << 21, 1 << 23, 1 << 24])
+@pytest.mark.parametrize("n", [1 << 17, 1 << 20, 1 << 21, 1 << 23, 1 << 24, 1 << 25])
 def test_r2c_full_size_sampled_bins_and_properties(torch, fd, orc, n):
-    """The paper's series lengths (2^20..2^24): sampled bins against direct sums, numpy's fp64 rfft
+    """The paper's series lengths (2^20..2^24) and the largest supported one (2^25): sampled bins against direct sums, numpy's fp64 rfft
     over the whole output as a third opinion, Parseval."""
     x = series(n, 7 + n % 1000, [(0.1 * n + 0.5, 10.0, 4.0)])
     got = run_r2c(torch, fd, x)

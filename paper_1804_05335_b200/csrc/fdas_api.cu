@@ -450,7 +450,7 @@ fdas_status fdas_harmonic_sum_threshold(fdas_plan *p, void *stream, const float 
     FDAS_CUDA(p, cudaMemsetAsync(d_count, 0, sizeof(uint64_t), st));
     const int nhalf = (I.ntemplates - 1) / 2, lim = nhalf / nharm;      // rows |z_k| <= zmax / H
     const long long nc = (I.ncols - 1) / nharm + 1;
-    const dim3 grid((unsigned)((nc + 255) / 256), (unsigned)(2 * lim + 1));
+    const dim3 grid((unsigned)((nc + 1023) / 1024), (unsigned)(2 * lim + 1));   // 4 columns per thread
     harmonic_sum_kernel<<<grid, 256, 0, st>>>(d_plane, I.ncols, I.ntemplates, nharm, nhalf - lim, threshold,
                                               (Candidate *)d_cands, capacity, (unsigned long long *)d_count);
     g_launches += 1;

@@ -207,25 +207,37 @@ __global__ void fp32_peak_kernel(float *out, int iters, float a, float b)
 }
 
 // Harmonic summing of a stored plane + threshold (fdas_harmonic_sum_threshold, include/fdas.h; PAPER.md:73, :79,
-// :331; reading R18): thread <-> fundamental column c of row blockIdx.y, S = sum_h P[row(h z_k)][h c].
+// :331; reading R18): S = sum_h P[row(h z_k)][h c] for the fundamental column c of row blockIdx.y.  A thread forms
+// four sums (columns c0 + {0, 1, 2, 3} * blockDim.x, so that every load of a warp is a run of consecutive addresses
+// with stride h) to keep 4 H independent loads in flight; the order of the additions is h = 1, 2, .. H.
 __global__ void __launch_bounds__(256) harmonic_sum_kernel(const float *__restrict__ plane, long long ncols, int K,
                                                            int nharm, int row_first, float threshold, Candidate *cands,
                                                            long long capacity, unsigned long long *count)
 {
-    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long nc = (ncols - 1) / nharm + 1;
-    if (c >= nc) return;
+    const long long c0 = (long long)blockIdx.x * (4 * blockDim.x) + threadIdx.x;
     const int k = row_first + blockIdx.y, center = (K - 1) / 2;
-    float s = 0.f;
-    for (int h = 1; h <= nharm; ++h) s += __ldg(plane + (size_t)(center + h * (k - center)) * ncols + h * c);
-    if (s > threshold) {
-        const unsigned long long slot = atomicAdd(count, 1ull);
-        if (slot < (unsigned long long)capacity) {
-            Candidate cd;
-            cd.col = c;
-            cd.row = k;
-            cd.power = s;
-            cands[slot] = cd;
+    float s[4] = {0.f, 0.f, 0.f, 0.f};
+    for (int h = 1; h <= nharm; ++h) {
+        const float *row = plane + (size_t)(center + h * (k - center)) * ncols;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const long long c = c0 + (long long)j * blockDim.x;
+            if (c < nc) s[j] += __ldg(row + h * c);
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const long long c = c0 + (long long)j * blockDim.x;
+        if (c < nc && s[j] > threshold) {
+            const unsigned long long slot = atomicAdd(count, 1ull);
+            if (slot < (unsigned long long)capacity) {
+                Candidate cd;
+                cd.col = c;
+                cd.row = k;
+                cd.power = s[j];
+                cands[slot] = cd;
+            }
         }
     }
 }

@@ -310,17 +310,31 @@ __device__ __forceinline__ void st_stream2_if(float *p, float a, float b, unsign
 // PAPER.md:73 "comparing the resulting Fourier power to a pre-calculated threshold", :331): the plane
 // never reaches memory; a cell above the threshold is appended to the candidate list (rare path:
 // its row / column are recovered from the address the store would have used).
-__device__ __noinline__ void push_candidate(const KernelParams &prm, const float *p, float v)
+// What the out-of-line candidate code needs, passed BY VALUE: taking the address of the kernel's parameter struct
+// for a call would make the compiler keep a copy of it in local memory and read every prm.x of the main loop from
+// there (measured in the interbinned threshold kernels: LDL + long-scoreboard waits on npairs, threshold, ...).
+struct CandSink {
+    const float *plane;
+    Candidate *cands;
+    unsigned long long *count;
+    long long capacity, ncols;
+    float threshold;
+};
+__device__ __forceinline__ CandSink sink_of(const KernelParams &prm)
 {
-    const long long idx = p - prm.plane;
-    const long long row = idx / prm.ncols;
-    const unsigned long long slot = atomicAdd(prm.count, 1ull);
-    if (slot < (unsigned long long)prm.capacity) {
+    return CandSink{prm.plane, prm.cands, prm.count, prm.capacity, prm.ncols, prm.threshold};
+}
+__device__ __noinline__ void push_candidate(const CandSink s, const float *p, float v)
+{
+    const long long idx = p - s.plane;
+    const long long row = idx / s.ncols;
+    const unsigned long long slot = atomicAdd(s.count, 1ull);
+    if (slot < (unsigned long long)s.capacity) {
         Candidate c;
-        c.col = idx - row * prm.ncols;
+        c.col = idx - row * s.ncols;
         c.row = (int)row;
         c.power = v;
-        prm.cands[slot] = c;
+        s.cands[slot] = c;
     }
 }
 template <int MODE>
@@ -329,7 +343,7 @@ __device__ __forceinline__ void emit_if(const KernelParams &prm, float *p, float
     if constexpr (MODE == 0) {
         st_stream_if(p, v, pred);
     } else {
-        if (pred && v > prm.threshold) push_candidate(prm, p, v);
+        if (pred && v > prm.threshold) push_candidate(sink_of(prm), p, v);
     }
 }
 template <int MODE>
@@ -338,8 +352,8 @@ __device__ __forceinline__ void emit2_if(const KernelParams &prm, float *p, floa
     if constexpr (MODE == 0) {
         st_stream2_if(p, a, b, pred);
     } else {
-        if (pred && a > prm.threshold) push_candidate(prm, p, a);
-        if (pred && b > prm.threshold) push_candidate(prm, p + 1, b);
+        if (pred && a > prm.threshold) push_candidate(sink_of(prm), p, a);
+        if (pred && b > prm.threshold) push_candidate(sink_of(prm), p + 1, b);
     }
 }
 
@@ -376,9 +390,16 @@ __device__ __forceinline__ void emit_cells(const KernelParams &prm, const cpk (&
 // MODE 1 slow path, out of line (its register needs and calls stay out of the main loop); entered by whole
 // warps only, so the interbin shuffles are converged.
 template <int L, bool INTERBIN, int STRIDE>
-__device__ __noinline__ void emit_cells_rare(const KernelParams &prm, const cpk (&y)[16], float *bp, float *bq,
+__device__ __noinline__ void emit_cells_rare(const CandSink s, const cpk (&y)[16], float *bp, float *bq,
                                              unsigned vm, unsigned vmq)
 {
+    KernelParams prm;                                   // the fields the candidate sink reads; local to the rare path
+    prm.plane = const_cast<float *>(s.plane);
+    prm.cands = s.cands;
+    prm.count = s.count;
+    prm.capacity = s.capacity;
+    prm.ncols = s.ncols;
+    prm.threshold = s.threshold;
     emit_cells<L, INTERBIN, 1, STRIDE>(prm, y, bp, bq, vm, vmq);
 }
 
@@ -409,7 +430,7 @@ __device__ __forceinline__ void emit_unit(const KernelParams &prm, const cpk (&y
             cpk ys[16];                              // a copy in local memory: y itself stays in registers
 #pragma unroll
             for (int n1 = 0; n1 < 16; ++n1) ys[n1] = y[n1];
-            emit_cells_rare<L, INTERBIN, STRIDE>(prm, ys, bp, bq, vm, vmq);
+            emit_cells_rare<L, INTERBIN, STRIDE>(sink_of(prm), ys, bp, bq, vm, vmq);
         }
     }
 }

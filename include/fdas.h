@@ -204,6 +204,43 @@ fdas_status fdas_r2c_execute(fdas_r2c_plan *plan, void *stream, const float *d_t
 /* Free the plan.  fdas_r2c_destroy(NULL) is a no-op returning FDAS_OK. */
 fdas_status fdas_r2c_destroy(fdas_r2c_plan *plan);
 
+/*
+ * The same transform for callers that may not allocate device memory.
+ *
+ * Who needs it: a host that cannot call cudaMalloc while it runs.  Examples are an acquisition back-end that split
+ * the card's memory once at start-up and must keep the allocator's device-wide lock, its implicit synchronisation
+ * and its possible failure (a neighbouring process filled the card) out of its real-time loop, and a plug-in inside
+ * a framework whose own memory pool already owns nearly all of the GPU, where an allocation made behind the
+ * framework's back fails or starves the framework.  Such a caller cannot use fdas_r2c_plan_create, which allocates.
+ *
+ * This call needs no plan and calls no cudaMalloc, cudaFree or allocating library routine, on its first call or any
+ * later one.  The work arrays and twiddle tables of the transform live in one array that is part of the library's
+ * device image: FDAS_R2C_STATIC_BYTES (8.04 MiB) on EVERY GPU that loads libfdas.so, held until the process exits
+ * whether or not this call is ever made.  That fixes the limit: nsamples must be a power of two with
+ * 2^10 <= nsamples <= FDAS_R2C_STATIC_MAX_SAMPLES (2^20); anything else returns FDAS_ERR_UNSUPPORTED, with the
+ * reason in fdas_last_error(NULL).  Longer series need fdas_r2c_plan_create.
+ *
+ *   stream, d_timeseries, d_spectrum, scale : as for fdas_r2c_execute (caller-owned input and output, nsamples
+ *                  float32 in, nsamples/2 complex64 out, 8- and 16-byte aligned, FDAS_ERR_ALIGNMENT otherwise).
+ *   result       : the same kernels with the same arguments as fdas_r2c_execute, so the same bits.
+ *
+ * First call on a device: looks up the array's address on the current device and raises the shared-memory limit of
+ * the transform kernels (host-side driver calls, no allocation).  Make that first call per device during start-up,
+ * before any stream capture begins.  A call whose nsamples differs from the previous call's on that device first
+ * refills the twiddle tables with five small launches on `stream`; otherwise it is the four launches of
+ * fdas_r2c_execute.  No host synchronisation.
+ *
+ * Sharing: all calls on a device use the one array, and it keeps whatever the last call left in it.  Nothing in
+ * it has to start at zero (every pass overwrites all it later reads), so back-to-back calls of any sizes on ONE
+ * stream are safe.  Two calls that can overlap on the GPU (different streams without an event between them,
+ * different host threads on different streams) race on the work arrays and tables and give wrong spectra silently;
+ * order them yourself.  Host-side the call is thread-safe (one mutex).
+ */
+#define FDAS_R2C_STATIC_MAX_SAMPLES (1ll << 20)
+#define FDAS_R2C_STATIC_BYTES (8ll * (FDAS_R2C_STATIC_MAX_SAMPLES + 3 * 256 + 4096 + FDAS_R2C_STATIC_MAX_SAMPLES / 4096))
+fdas_status fdas_r2c_execute_static(void *stream, const float *d_timeseries, int64_t nsamples, void *d_spectrum,
+                                    float scale);
+
 /* ---- introspection for harnesses and tests (not on the hot path) ---- */
 
 fdas_status fdas_plan_info(const fdas_plan *plan, fdas_info *out);
@@ -235,7 +272,7 @@ int64_t fdas_launch_count(void);
 
 const char *fdas_status_string(fdas_status s);
 /* Text of the last CUDA error seen by this plan ("" if none); plan = NULL: of the calling thread's last
- * failed fdas_plan_create. */
+ * failed fdas_plan_create, fdas_r2c_plan_create or fdas_r2c_execute_static. */
 const char *fdas_last_error(const fdas_plan *plan);
 
 #ifdef __cplusplus

@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -656,6 +657,130 @@ fdas_status fdas_r2c_destroy(fdas_r2c_plan *p)
     cudaGetLastError();
     delete p;
     return FDAS_OK;
+}
+
+// ---------------------------------------------------------------- the transform for callers that may not allocate
+} // extern "C"
+
+// fdas_r2c_execute_static (include/fdas.h) is for hosts that cannot call cudaMalloc while they run: an acquisition
+// back-end that divided the card's memory once at start-up and must not take the allocator's device-wide lock (or
+// its failure when a neighbour has filled the card) inside its real-time loop, or a plug-in living inside a
+// framework whose own pool already holds nearly all of HBM.  For them everything the transform needs beyond its
+// input and output -- the two work arrays between the passes and the five twiddle tables -- lives in ONE
+// file-scope device array, which every GPU that loads libfdas.so holds from module load until the process exits
+// (8.04 MiB; nothing is ever freed).  Layout in float2 elements:
+//     [0, MAXM) work 0 | [MAXM, 2 MAXM) work 1 | 3 x 256 exp(-2 pi i j / N_i) | 4096 t_lo | 256 t_hi
+// Every sub-array starts on a 256-byte boundary.  Host code may not hand `g_r2c_static_scratch` itself to a
+// kernel: on the host that name is only a handle for the symbol; its device address comes from
+// cudaGetSymbolAddress, taken once per device (below) with that device current.
+constexpr long long R2C_STATIC_MAXM = FDAS_R2C_STATIC_MAX_SAMPLES / 2;
+constexpr long long R2C_STATIC_ELEMS = 2 * R2C_STATIC_MAXM + 3 * 256 + 4096 + FDAS_R2C_STATIC_MAX_SAMPLES / 4096;
+static __device__ __align__(256) float2 g_r2c_static_scratch[R2C_STATIC_ELEMS];
+static_assert(sizeof(float2) * R2C_STATIC_ELEMS == FDAS_R2C_STATIC_BYTES, "fdas.h states the size of the static scratch array");
+
+namespace {
+
+constexpr int R2C_STATIC_MAX_DEVICES = 64;
+
+struct R2CStaticDevice {
+    bool ready;            // address taken and kernel attributes set on this device
+    fdas_r2c_plan plan;    // a plan whose pointers all lie inside g_r2c_static_scratch; plan.n = size of the tables
+};
+R2CStaticDevice g_r2c_static_dev[R2C_STATIC_MAX_DEVICES];   // zero-initialised
+std::mutex g_r2c_static_mutex;
+
+} // namespace
+
+extern "C" {
+
+fdas_status fdas_r2c_execute_static(void *stream, const float *d_timeseries, int64_t nsamples, void *d_spectrum,
+                                    float scale)
+{
+    if (!d_timeseries || !d_spectrum || nsamples <= 0) return FDAS_ERR_INVALID_ARG;
+    int p2 = 0;
+    while (p2 < 62 && (1ll << p2) < nsamples) ++p2;
+    if ((1ll << p2) != nsamples || p2 < 10 || nsamples > FDAS_R2C_STATIC_MAX_SAMPLES) {
+        snprintf(g_create_err, sizeof(g_create_err),
+                 "fdas_r2c_execute_static: nsamples = %lld; needs a power of two in [1024, %lld] (the static scratch "
+                 "array holds no more; longer series need fdas_r2c_plan_create)",
+                 (long long)nsamples, (long long)FDAS_R2C_STATIC_MAX_SAMPLES);
+        return FDAS_ERR_UNSUPPORTED;
+    }
+    if (((uintptr_t)d_timeseries & 7) || ((uintptr_t)d_spectrum & 15)) return FDAS_ERR_ALIGNMENT;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess && (dev < 0 || dev >= R2C_STATIC_MAX_DEVICES)) {
+        snprintf(g_create_err, sizeof(g_create_err), "fdas_r2c_execute_static: device ordinal %d not supported", dev);
+        return FDAS_ERR_UNSUPPORTED;
+    }
+    if (e != cudaSuccess) {
+        snprintf(g_create_err, sizeof(g_create_err), "fdas_r2c_execute_static: %s", cudaGetErrorString(e));
+        cudaGetLastError();
+        return FDAS_ERR_CUDA;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    std::lock_guard<std::mutex> lock(g_r2c_static_mutex);
+    R2CStaticDevice &D = g_r2c_static_dev[dev];
+    fdas_r2c_plan &P = D.plan;
+    if (!D.ready) {
+        // Once per device, with that device current: the array's address ON THIS DEVICE, and the shared-memory
+        // limit of the two transform kernels (a per-device function attribute).  Neither allocates.
+        float2 *base = nullptr;
+        e = cudaGetSymbolAddress((void **)&base, g_r2c_static_scratch);
+        for (const void *k : {(const void *)r2c_cols_kernel, (const void *)r2c_rows_kernel})
+            if (e == cudaSuccess)
+                e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (8192 + 32 + 256) * 8);
+        if (e != cudaSuccess || !base) {
+            snprintf(g_create_err, sizeof(g_create_err), "fdas_r2c_execute_static: set-up on device %d: %s", dev,
+                     e != cudaSuccess ? cudaGetErrorString(e) : "null symbol address");
+            cudaGetLastError();
+            return FDAS_ERR_CUDA;
+        }
+        std::memset(&P, 0, sizeof(P));
+        P.device = dev;
+        P.d_work[0] = base;
+        P.d_work[1] = base + R2C_STATIC_MAXM;
+        for (int i = 0; i < 3; ++i) P.d_w[i] = base + 2 * R2C_STATIC_MAXM + 256 * i;
+        P.d_tlo = P.d_w[2] + 256;
+        P.d_thi = P.d_tlo + 4096;
+        D.ready = true;
+    }
+    if (P.n != nsamples) {
+        // Another length than the last call on this device: same factorisation rule as fdas_r2c_plan_create, and
+        // the tables are refilled ON THE CALLER'S STREAM, behind whatever that stream still has to do with the old
+        // ones.  (The work arrays need no clearing: every pass writes all M elements before the next reads them.)
+        const int lm = p2 - 1;
+        P.lg[0] = lm / 3;
+        P.lg[1] = (lm - P.lg[0]) / 2;
+        P.lg[2] = lm - P.lg[0] - P.lg[1];
+        auto ltile_for = [](int log2R, int log2avail) {
+            int t = 5;
+            if (t > log2avail) t = log2avail;
+            if (t > 13 - log2R) t = 13 - log2R;
+            return t;
+        };
+        P.lt[0] = ltile_for(P.lg[0], P.lg[1] + P.lg[2]);
+        P.lt[1] = ltile_for(P.lg[1], P.lg[2]);
+        P.lt[2] = ltile_for(P.lg[2], P.lg[0]);
+        P.n = 0;                                              // tables invalid until all five launches are queued
+        P.M = nsamples / 2;
+        const long long nhi = (nsamples + 4095) / 4096;
+        for (int i = 0; i < 3; ++i) {
+            const long long R = 1ll << P.lg[i];
+            r2c_table_kernel<<<(unsigned)((R + 127) / 128), 128, 0, st>>>(P.d_w[i], R, 1, R);
+        }
+        r2c_table_kernel<<<32, 128, 0, st>>>(P.d_tlo, 4096, 1, nsamples);
+        r2c_table_kernel<<<(unsigned)((nhi + 127) / 128), 128, 0, st>>>(P.d_thi, nhi, 4096, nsamples);
+        g_launches += 5;
+        e = cudaGetLastError();
+        if (e != cudaSuccess) {
+            snprintf(g_create_err, sizeof(g_create_err), "fdas_r2c_execute_static: twiddle tables: %s",
+                     cudaGetErrorString(e));
+            return FDAS_ERR_CUDA;
+        }
+        P.n = nsamples;
+    }
+    return fdas_r2c_execute(&P, stream, d_timeseries, d_spectrum, scale);   // the four passes, unchanged
 }
 
 fdas_status fdas_measure_fp32_peak(void *stream, int32_t iters, double *tflops)

@@ -23,7 +23,10 @@ EXPORTS = ["fdas_plan_create", "fdas_make_templates", "fdas_execute", "fdas_exec
            "fdas_destroy",
            "fdas_plan_info", "fdas_get_taps", "fdas_get_template_spectrum", "fdas_measure_fp32_peak",
            "fdas_launch_count", "fdas_status_string", "fdas_last_error",
-           "fdas_harmonic_sum_threshold", "fdas_r2c_plan_create", "fdas_r2c_execute", "fdas_r2c_destroy"]
+           "fdas_harmonic_sum_threshold", "fdas_r2c_plan_create", "fdas_r2c_execute", "fdas_r2c_destroy",
+           "fdas_r2c_execute_static"]
+
+R2C_STATIC_MAX_SAMPLES = 1 << 20      # FDAS_R2C_STATIC_MAX_SAMPLES of include/fdas.h
 
 
 class FdasInfo(ctypes.Structure):
@@ -64,6 +67,7 @@ def _load() -> ctypes.CDLL:
     lib.fdas_r2c_plan_create.argtypes = [ctypes.POINTER(vp), i64]
     lib.fdas_r2c_execute.argtypes = [vp, vp, vp, vp, ctypes.c_float]
     lib.fdas_r2c_destroy.argtypes = [vp]
+    lib.fdas_r2c_execute_static.argtypes = [vp, vp, i64, vp, ctypes.c_float]
     lib.fdas_plan_info.argtypes = [vp, ctypes.POINTER(FdasInfo)]
     lib.fdas_get_taps.argtypes = [vp, i32, vp, ctypes.POINTER(i32)]
     lib.fdas_get_template_spectrum.argtypes = [vp, i32, vp]
@@ -167,6 +171,15 @@ def fdas_r2c_execute(plan: int, stream, d_timeseries, d_spectrum, scale: float =
 
 def fdas_r2c_destroy(plan: int) -> None:
     _check(lib.fdas_r2c_destroy(plan), "fdas_r2c_destroy")
+
+
+def fdas_r2c_execute_static(stream, d_timeseries, nsamples: int, d_spectrum, scale: float = 1.0) -> None:
+    """The transform of fdas_r2c_execute without a plan and without any device allocation, for callers that may not
+    call cudaMalloc (a real-time loop, a host whose memory pool owns the GPU): its scratch is a fixed array inside the
+    library, so nsamples <= R2C_STATIC_MAX_SAMPLES, and calls that overlap on the GPU race (include/fdas.h)."""
+    st = lib.fdas_r2c_execute_static(_stream(stream), _ptr(d_timeseries), int(nsamples), _ptr(d_spectrum), float(scale))
+    if st != FDAS_OK:
+        raise FdasError(st, "fdas_r2c_execute_static", lib.fdas_last_error(None).decode() if st in (2, 5) else "")
 
 
 def fdas_destroy(plan: int) -> None:

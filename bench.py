@@ -414,7 +414,6 @@ def time_r2c(torch, fdas, dev, stream, n, peaks, steps=20):
     gbs = 8.0 * n / (ms * 1e-3) / 1e9
     return {"nsamples": n, "ms": ms, "samples_per_s": n / (ms * 1e-3), "launches_per_call": 4,
             "alg_bytes": 8 * n, "design_bytes": 32 * n, "achieved_gbs": gbs, "frac_hbm": gbs / peaks["hbm_gbs"],
-            "frac_hbm_of_design_traffic": 4.0 * gbs / peaks["hbm_gbs"],
             "l2": "working set (series + 2 work arrays + spectrum) = %d MB: %s the 126 MB L2 between passes and calls"
                   % (16 * n >> 20, "stays in" if 16 * n < (120 << 20) else "larger than")}
 

@@ -65,7 +65,10 @@ typedef struct fdas_info {
     int32_t npairs;       /* (K+1)/2 template slots processed by the kernel (+-z share one slot)      */
     int32_t threads;      /* threads per CTA of the fused kernel                                     */
     int32_t grid;         /* CTAs launched by fdas_execute (persistent; multiple of the SM count)    */
-    int32_t ctas_per_sm;  /* resident CTAs per SM the grid was sized for                             */
+    int32_t ctas_per_sm;  /* resident CTAs per SM the grid was sized for: the occupancy API's answer, or, for
+                             the tensor-memory kernel of seglen 2048 (where that API answers 1), the number
+                             worked out from the compiled kernels' registers and shared memory and the
+                             device's limits (3 on a B200; smaller if fewer fit, never assumed)          */
     int32_t smem_bytes;   /* dynamic shared memory per CTA                                           */
     int32_t regs;         /* registers per thread of the fused kernel                                */
     int32_t sm_count;     /* SMs on the device                                                       */
@@ -165,8 +168,10 @@ fdas_status fdas_execute_threshold_host(fdas_plan *plan, void *stream, const voi
  *   d_plane : device, the ntemplates x ncols float32 plane fdas_execute wrote (read only), 16-byte aligned.
  *   nharm   : H >= 1 (searches usually sum 2, 4, 8, 16 harmonics in turn; call once per H).
  *   d_cands / capacity / d_count : as for fdas_execute_threshold (d_count is zeroed on `stream` first).
- * Errors: FDAS_ERR_INVALID_ARG (null pointers, nharm < 1, NaN threshold, capacity < 0), FDAS_ERR_ALIGNMENT,
- * FDAS_ERR_CUDA.  Needs no templates (works on any plane of the plan's shape).
+ * Errors: FDAS_ERR_INVALID_ARG (null pointers, nharm < 1, NaN threshold, capacity < 0), FDAS_ERR_ALIGNMENT (d_cands
+ * is checked only when capacity > 0: it is never written otherwise), FDAS_ERR_UNSUPPORTED (rows x ceil(columns /
+ * 1024) beyond 2^31 - 1 CTAs; any bank size is fine otherwise), FDAS_ERR_CUDA.  Needs no templates (works on any
+ * plane of the plan's shape).
  */
 fdas_status fdas_harmonic_sum_threshold(fdas_plan *plan, void *stream, const float *d_plane, int32_t nharm,
                                         float threshold, fdas_candidate *d_cands, int64_t capacity,
@@ -197,6 +202,10 @@ fdas_status fdas_r2c_plan_create(fdas_r2c_plan **out, int64_t nsamples);
  *                  handed to fdas_execute of a plan with nbins = nsamples/2 on the same stream.
  *   scale        : multiplies every bin (1/nsamples-type normalisations are the caller's choice; the paper's
  *                  pipeline normalises the spectrum outside the part it covers).
+ * One plan, one stream at a time: the plan's two work arrays are shared by all of its calls, so two calls on the
+ * same plan that can overlap on the GPU (different streams with no event between them) race silently.  Calls on
+ * one stream, or on separate plans, are safe.  Errors: FDAS_ERR_INVALID_ARG (null pointers, another device
+ * current than the plan's), FDAS_ERR_ALIGNMENT, FDAS_ERR_CUDA.
  */
 fdas_status fdas_r2c_execute(fdas_r2c_plan *plan, void *stream, const float *d_timeseries, void *d_spectrum,
                              float scale);

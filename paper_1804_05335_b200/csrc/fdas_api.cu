@@ -4,6 +4,7 @@
 #include "../../include/fdas.h"
 #include "fdas_templates.cuh"
 
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdio>
@@ -100,7 +101,7 @@ kernel_fn pick_kernel3(int ib, int mode)
 constexpr int K3_CTAS_PER_SM_2048 = 3;   // fdas_kernel3.cuh at L = 2048: <= 168 registers, 72 KB, 128 tensor-memory columns
 
 // mode 0: plane store (fdas_execute); mode 1: threshold search (fdas_execute_threshold)
-// ib: 0 none, 1 interbinning (eq. 4), 2 two-bin Fourier interpolation (second template bank; L <= 4096)
+// ib: 0 none, 1 interbinning (eq. 4), 2 two-bin Fourier interpolation (second template bank)
 kernel_fn select_kernel(int L, int ib, int mode = 0)
 {
     switch (L) {
@@ -125,6 +126,32 @@ int smem_bytes_for(int L, bool ib)
     case 8192: return Geo8k::smem_bytes();
     default: return 0;
     }
+}
+
+// Tensor-memory columns one CTA of the selected kernel allocates (0: none).  L = 4096 runs without parking.
+int tmem_cols_for(int L)
+{
+    switch (L) {
+    case 2048: return Geo3<2048>::TM_COLS;
+    case 8192: return Geo8k::TM_COLS;
+    default: return 0;
+    }
+}
+
+// CTAs of one kernel an SM can hold at once, from the device's limits: registers (allocated per warp in units of 8
+// per thread), shared memory (dynamic + static + the per-CTA reserve), the 512 tensor-memory columns, threads and
+// CTA slots.  cudaOccupancyMaxActiveBlocksPerMultiprocessor cannot be asked: it answers 1 for every kernel that
+// allocates tensor memory.
+int resident_ctas(const cudaDeviceProp &prop, const cudaFuncAttributes &fa, int threads, int smem_dyn, int tm_cols)
+{
+    const long long regs_cta = (long long)((fa.numRegs + 7) / 8 * 8) * ((threads + 31) / 32 * 32);
+    const long long smem_cta = (long long)smem_dyn + (long long)fa.sharedSizeBytes + (long long)prop.reservedSharedMemPerBlock;
+    long long n = prop.maxBlocksPerMultiProcessor;
+    if (regs_cta > 0 && prop.regsPerMultiprocessor / regs_cta < n) n = prop.regsPerMultiprocessor / regs_cta;
+    if (smem_cta > 0 && (long long)prop.sharedMemPerMultiprocessor / smem_cta < n) n = (long long)prop.sharedMemPerMultiprocessor / smem_cta;
+    if (tm_cols > 0 && 512 / tm_cols < n) n = 512 / tm_cols;
+    if (prop.maxThreadsPerMultiProcessor / threads < n) n = prop.maxThreadsPerMultiProcessor / threads;
+    return (int)n;
 }
 
 void freq_to_reg_any(int L, int f, int &tid, int &i)
@@ -245,8 +272,18 @@ fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double
         if (occ < 1) { st = FDAS_ERR_UNSUPPORTED; break; }
         // cudaOccupancyMaxActiveBlocksPerMultiprocessor answers 1 for any kernel that uses tensor memory
         // (EIATTR_TCGEN05_1CTA_USED); fdas_kernel3.cuh allocates 128 of the SM's 512 columns per CTA and is
-        // built for K3_CTAS_PER_SM_2048 CTAs per SM by registers and shared memory (measured: they are co-resident).
-        if (seglen == 2048 && occ < K3_CTAS_PER_SM_2048) occ = K3_CTAS_PER_SM_2048;
+        // built for K3_CTAS_PER_SM_2048 CTAs per SM.  Whether that many really fit is worked out here from the
+        // compiled kernels' registers and shared memory and the device's limits, for BOTH kernels that share the
+        // grid; if fewer fit (another device, a later edit that costs registers) the persistent grid shrinks with it
+        // instead of leaving a third of the CTAs to run as a serial tail, and fdas_info reports the smaller number.
+        if (seglen == 2048 && occ < K3_CTAS_PER_SM_2048) {
+            cudaFuncAttributes fb;
+            if ((e = cudaFuncGetAttributes(&fb, (const void *)p->kernel_thr)) != cudaSuccess) FDAS_CREATE_FAIL(FDAS_ERR_CUDA)
+            const int tm = tmem_cols_for(seglen);
+            const int fit = std::min(resident_ctas(prop, fa, I.threads, I.smem_bytes, tm),
+                                     resident_ctas(prop, fb, I.threads, I.smem_bytes, tm));
+            occ = std::max(occ, std::min(fit, K3_CTAS_PER_SM_2048));
+        }
         I.ctas_per_sm = occ;
         I.grid = occ * I.sm_count;
         const size_t taps_bytes = (size_t)p->nbanks * K * (2 * m + 1) * sizeof(double2);
@@ -363,8 +400,8 @@ fdas_status fdas_execute_threshold(fdas_plan *p, void *stream, const void *d_spe
         !on_plan_device(p))
         return FDAS_ERR_INVALID_ARG;
     if (!p->ready) return FDAS_ERR_NOT_READY;
-    if (((uintptr_t)d_spectrum & 15) || ((uintptr_t)d_cands & 15) || ((uintptr_t)d_count & 7))
-        return FDAS_ERR_ALIGNMENT;
+    if (((uintptr_t)d_spectrum & 15) || (capacity > 0 && ((uintptr_t)d_cands & 15)) || ((uintptr_t)d_count & 7))
+        return FDAS_ERR_ALIGNMENT;   // d_cands is never written when capacity is 0
     FDAS_CUDA(p, cudaMemsetAsync(d_count, 0, sizeof(uint64_t), (cudaStream_t)stream));
     return launch_fused(p, stream, d_spectrum, nullptr, threshold, d_cands, capacity,
                         (unsigned long long *)d_count);
@@ -445,15 +482,22 @@ fdas_status fdas_harmonic_sum_threshold(fdas_plan *p, void *stream, const float 
     if (!p || !d_plane || !d_count || nharm < 1 || capacity < 0 || (capacity > 0 && !d_cands) ||
         threshold != threshold || !on_plan_device(p))
         return FDAS_ERR_INVALID_ARG;
-    if (((uintptr_t)d_plane & 15) || ((uintptr_t)d_cands & 15) || ((uintptr_t)d_count & 7)) return FDAS_ERR_ALIGNMENT;
+    if (((uintptr_t)d_plane & 15) || (capacity > 0 && ((uintptr_t)d_cands & 15)) || ((uintptr_t)d_count & 7))
+        return FDAS_ERR_ALIGNMENT;
     const fdas_info &I = p->info;
     cudaStream_t st = (cudaStream_t)stream;
     FDAS_CUDA(p, cudaMemsetAsync(d_count, 0, sizeof(uint64_t), st));
     const int nhalf = (I.ntemplates - 1) / 2, lim = nhalf / nharm;      // rows |z_k| <= zmax / H
     const long long nc = (I.ncols - 1) / nharm + 1;
-    const dim3 grid((unsigned)((nc + 1023) / 1024), (unsigned)(2 * lim + 1));   // 4 columns per thread
-    harmonic_sum_kernel<<<grid, 256, 0, st>>>(d_plane, I.ncols, I.ntemplates, nharm, nhalf - lim, threshold,
-                                              (Candidate *)d_cands, capacity, (unsigned long long *)d_count);
+    // one CTA per (row, block of 1024 columns), rows folded into blockIdx.x: grid.y would cap the bank at 65 535 rows
+    const long long nbx = (nc + 1023) / 1024, nblocks = nbx * (2 * lim + 1);    // 4 columns per thread
+    if (nblocks > 0x7fffffffll) {
+        snprintf(p->err, sizeof(p->err), "fdas_harmonic_sum_threshold: %lld CTAs exceed the grid limit", nblocks);
+        return FDAS_ERR_UNSUPPORTED;
+    }
+    harmonic_sum_kernel<<<(unsigned)nblocks, 256, 0, st>>>(d_plane, I.ncols, I.ntemplates, nharm, nhalf - lim,
+                                                           (unsigned)nbx, threshold, (Candidate *)d_cands, capacity,
+                                                           (unsigned long long *)d_count);
     g_launches += 1;
     FDAS_CUDA(p, cudaGetLastError());
     return FDAS_OK;

@@ -207,16 +207,19 @@ __global__ void fp32_peak_kernel(float *out, int iters, float a, float b)
 }
 
 // Harmonic summing of a stored plane + threshold (fdas_harmonic_sum_threshold, include/fdas.h; PAPER.md:73, :79,
-// :331; reading R18): S = sum_h P[row(h z_k)][h c] for the fundamental column c of row blockIdx.y.  A thread forms
+// :331; reading R18): S = sum_h P[row(h z_k)][h c] for the fundamental column c of row blockIdx.x / nbx (column
+// block blockIdx.x % nbx; rows are folded into x because gridDim.y stops at 65 535).  A thread forms
 // four sums (columns c0 + {0, 1, 2, 3} * blockDim.x, so that every load of a warp is a run of consecutive addresses
 // with stride h) to keep 4 H independent loads in flight; the order of the additions is h = 1, 2, .. H.
 __global__ void __launch_bounds__(256) harmonic_sum_kernel(const float *__restrict__ plane, long long ncols, int K,
-                                                           int nharm, int row_first, float threshold, Candidate *cands,
-                                                           long long capacity, unsigned long long *count)
+                                                           int nharm, int row_first, unsigned nbx, float threshold,
+                                                           Candidate *cands, long long capacity,
+                                                           unsigned long long *count)
 {
     const long long nc = (ncols - 1) / nharm + 1;
-    const long long c0 = (long long)blockIdx.x * (4 * blockDim.x) + threadIdx.x;
-    const int k = row_first + blockIdx.y, center = (K - 1) / 2;
+    const unsigned by = blockIdx.x / nbx, bx = blockIdx.x - by * nbx;
+    const long long c0 = (long long)bx * (4 * blockDim.x) + threadIdx.x;
+    const int k = row_first + (int)by, center = (K - 1) / 2;
     float s[4] = {0.f, 0.f, 0.f, 0.f};
     for (int h = 1; h <= nharm; ++h) {
         const float *row = plane + (size_t)(center + h * (k - center)) * ncols;

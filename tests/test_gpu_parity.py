@@ -406,6 +406,21 @@ def test_segmentation_independence_on_gpu(torch, fd, syn):
     assert np.max(np.abs(a - c)) < 2e-5 * np.max(a)
 
 
+@pytest.mark.parametrize("interbin", [0, 1, 2])
+def test_seglen_2048_grid_is_sized_from_computed_residency(torch, fd, interbin):
+    """The 2048 kernel is built for three CTAs per SM; the occupancy API cannot confirm that for a tensor-memory
+    kernel, so fdas_plan_create works it out from registers, shared memory and tensor-memory columns.
+    On a B200 the answer must be 3 -- a later edit that costs registers or shared memory fails here instead of
+    silently running a third of the grid as a serial tail."""
+    with fd.Plan(1 << 16, 84.0, 2.0, 2048, interbin) as plan:
+        I = plan.info
+        prop = torch.cuda.get_device_properties(0)
+        assert I.sm_count == prop.multi_processor_count
+        assert I.ctas_per_sm == 3 and I.grid == 3 * I.sm_count
+        assert ((I.regs + 7) // 8 * 8) * I.threads * 3 <= prop.regs_per_multiprocessor
+        assert 3 * (I.smem_bytes + 1024) <= prop.shared_memory_per_multiprocessor
+
+
 def test_error_codes_on_device(torch, fd):
     with fd.Plan(4096, 20.0, 2.0, 1024, 0) as plan:
         spec = torch.zeros(4096, 2, device="cuda")

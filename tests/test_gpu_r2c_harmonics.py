@@ -219,3 +219,51 @@ def test_harmonic_sum_errors(torch, fd):
         plan.harmonic_sum_threshold(None, d_plane, 64, -1.0, d_cands, 16, d_count)     # H > nhalf: the z = 0 row only
         torch.cuda.synchronize()
         assert int(d_count.item()) == (4096 - 1) // 64 + 1
+        # capacity 0 counts only: the candidate pointer is never written, so its alignment is not checked
+        plan.harmonic_sum_threshold(None, d_plane, 1, -1.0, d_cands[8:], 0, d_count)
+        torch.cuda.synchronize()
+        assert int(d_count.item()) == 21 * 4096
+        with pytest.raises(fd.FdasError) as e:
+            plan.harmonic_sum_threshold(None, d_plane, 1, -1.0, d_cands[8:], 4, d_count)
+        assert e.value.status == 4
+
+
+@pytest.mark.parametrize("nharm", [1, 2, 5])
+def test_harmonic_sum_bank_of_more_than_65535_rows(torch, fd, orc, nharm):
+    """A bank finer than any BASELINE config (dz = 0.001: 70 001 rows) is legal for fdas_plan_create; the harmonic
+    search must take it (rows used to sit in gridDim.y, which stops at 65 535: ADVICE r2).  Random exponential
+    powers stand in for a plane; the sums are compared exactly with float32 sums in the kernel's order and with the
+    oracle's fp64 sums."""
+    zmax, dz, ncols = 35.0, 0.001, 300
+    with fd.Plan(ncols, zmax, dz, 1024, 0) as plan:
+        K = plan.info.ntemplates
+        assert K == 70001 and plan.info.ncols == ncols
+        rng = np.random.Generator(np.random.Philox(4242))
+        plane = rng.standard_exponential((K, ncols)).astype(np.float32)
+        d_plane = torch.from_numpy(plane).cuda()
+        cap = 1 << 20
+        d_cands = torch.zeros(cap * 16, dtype=torch.uint8, device="cuda")
+        d_count = torch.zeros(1, dtype=torch.int64, device="cuda")
+        thr = nharm + 3.0 * math.sqrt(nharm) + 2.0
+        plan.harmonic_sum_threshold(torch.cuda.current_stream(), d_plane, nharm, thr, d_cands, cap, d_count)
+        torch.cuda.synchronize()
+        got = read_cands(torch, d_cands, d_count, cap)
+    rows = orc.harmonic_rows(zmax, dz, nharm)
+    assert rows.size == 2 * (35000 // nharm) + 1
+    nhalf, nc = (K - 1) // 2, (ncols - 1) // nharm + 1
+    s32 = np.zeros((rows.size, nc), dtype=np.float32)
+    for h in range(1, nharm + 1):
+        s32 += plane[nhalf + h * (rows - nhalf)][:, 0:h * (nc - 1) + 1:h]
+    ii, cc = np.nonzero(s32 > np.float32(thr))
+    assert got.size == ii.size > 1000
+    assert np.array_equal(got["row"], rows[ii]) and np.array_equal(got["col"], cc)
+    assert np.array_equal(got["power"], s32[ii, cc])
+    if nharm == 1:
+        assert rows.size > 65535 and got["row"].max() > 65535     # the case gridDim.y could not hold
+    s64 = orc.harmonic_sum(plane, zmax, dz, nharm)
+    assert np.max(np.abs(s32 - s64)) <= 1e-5 * s64.max()
+    r_o, c_o, _ = orc.harmonic_candidates(plane, zmax, dz, nharm, thr)
+    near = np.abs(s64 - thr) < 1e-5 * thr
+    index_of = {int(r): i for i, r in enumerate(rows)}
+    for (rr, c_) in set(zip(r_o.tolist(), c_o.tolist())) ^ set(zip(got["row"].tolist(), got["col"].tolist())):
+        assert near[index_of[rr], c_], (rr, c_)

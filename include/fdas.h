@@ -84,6 +84,10 @@ typedef struct fdas_info {
  * Fourier interpolation (a second template bank, twice the transforms), any seglen.
  * Allocates the plan-owned device memory (taps, template spectra, twiddle table).
  * *out is set to NULL on failure.
+ * Debug aid: with the environment variable FDAS_DEBUG_E1_SYNC=1 at the time of this call, a seglen-8192 plan's
+ * fdas_execute runs a build of its kernel with a CTA barrier in front of every store into the shared exchange
+ * buffer (the hand-shake the shipped kernel replaces by an ordering argument).  Same bits, a few per cent slower;
+ * a difference between the two planes points at a race in the shipped kernel.
  */
 fdas_status fdas_plan_create(fdas_plan **out, int64_t nbins, double zmax, double dz,
                              int32_t seglen, int32_t interbin);
@@ -281,7 +285,7 @@ int64_t fdas_launch_count(void);
 
 const char *fdas_status_string(fdas_status s);
 /* Text of the last CUDA error seen by this plan ("" if none); plan = NULL: of the calling thread's last
- * failed fdas_plan_create, fdas_r2c_plan_create or fdas_r2c_execute_static. */
+ * failed fdas_plan_create, fdas_r2c_plan_create, fdas_r2c_execute or fdas_r2c_execute_static. */
 const char *fdas_last_error(const fdas_plan *plan);
 
 #ifdef __cplusplus

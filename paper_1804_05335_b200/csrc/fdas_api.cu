@@ -104,6 +104,14 @@ constexpr int K3_CTAS_PER_SM_2048 = 3;   // fdas_kernel3.cuh at L = 2048: <= 168
 // ib: 0 none, 1 interbinning (eq. 4), 2 two-bin Fourier interpolation (second template bank)
 kernel_fn select_kernel(int L, int ib, int mode = 0)
 {
+    // debug aid (include/fdas.h, fdas_plan_create): the 8192 plane kernels with a CTA barrier in front of every E1 store
+    if (L == 8192 && mode == 0) {
+        const char *dbg = std::getenv("FDAS_DEBUG_E1_SYNC");
+        if (dbg && dbg[0] == '1') {
+            if (ib == 2) return (kernel_fn)fdas_fused_kernel_8k<1, 0, false, 2, true>;
+            return ib ? (kernel_fn)fdas_fused_kernel_8k<1, 0, true, 1, true> : (kernel_fn)fdas_fused_kernel_8k<1, 0, false, 1, true>;
+        }
+    }
     switch (L) {
     case 1024: return pick_kernel<1024, 4>(ib, mode);
     case 2048: return pick_kernel3<2048, K3_CTAS_PER_SM_2048>(ib, mode);
@@ -687,7 +695,11 @@ fdas_status fdas_r2c_execute(fdas_r2c_plan *p, void *stream, const float *d_time
     r2c_rows_kernel<<<dim3((unsigned)(N1 >> p->lt[2]), (unsigned)N2), R2C_THREADS, smem(p->lg[2], p->lt[2]), st>>>(q);
     r2c_untangle_kernel<<<(unsigned)((p->M / 2 + 1 + 255) / 256), 256, 0, st>>>(q);
     g_launches += 4;
-    if (cudaGetLastError() != cudaSuccess) return FDAS_ERR_CUDA;
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {                                   // the r2c plan has no text buffer: fdas_last_error(NULL)
+        snprintf(g_create_err, sizeof(g_create_err), "fdas_r2c_execute: %s", cudaGetErrorString(e));
+        return FDAS_ERR_CUDA;
+    }
     return FDAS_OK;
 }
 

@@ -130,7 +130,10 @@ __device__ __forceinline__ void store_rows_8k(const cpk (&y)[16], float *bp, flo
 // BANKS = 2 (two-bin Fourier interpolation, reading R16; plain sub-units only): prm.npairs counts
 // template SLOTS, slot = 2 * pair + bank, as in fdas_kernel.cuh: bank 0 fills the even plane columns, bank 1 (the
 // templates at half-integer offsets) the odd ones, and bank 1's q transform is the +|z| row shifted by one bin.
-template <int MINB, int MODE = 0, bool INTERBIN = false, int BANKS = 1>
+// ESYNC (debug, FDAS_DEBUG_E1_SYNC=1 at fdas_plan_create): a CTA barrier in front of every E1 store, i.e. the
+// `empty` hand-shake the two-buffer ordering argument below replaces.  A plane that differs between the two
+// builds means that argument no longer holds (tests/test_gpu_parity.py::test_seglen_8192_matches_its_e1_sync_build).
+template <int MINB, int MODE = 0, bool INTERBIN = false, int BANKS = 1, bool ESYNC = false>
 __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelParams prm)
 {
     using G = Geo<4096>;
@@ -264,7 +267,10 @@ __global__ void __launch_bounds__(256, MINB) fdas_fused_kernel_8k(const KernelPa
 #pragma unroll
             for (int n2 = 0; n2 < 16; ++n2) a[n2] = cmul(a[n2], tw.tw2[n2]);
             // E1[c & 1]: every warp finished loading sub-unit c-2 from it before it arrived for c-1, and this
-            // warp has waited for c-1's arrivals -- no `empty` barrier with two buffers
+            // warp has waited for c-1's arrivals -- no `empty` barrier with two buffers.  This holds only while the
+            // y[] loads of a sub-unit stay in front of the next mbar_arrive in program order and the segment-start
+            // path keeps its leading __syncthreads; ESYNC re-creates the barrier to check that mechanically.
+            if constexpr (ESYNC) __syncthreads();
 #pragma unroll
             for (int n2 = 0; n2 < 16; ++n2) e1.put(tm.e1_q2 + n2 * G::R3, a[n2]);
         }

@@ -165,8 +165,9 @@ def fdas_r2c_plan_create(nsamples: int) -> int:
 
 
 def fdas_r2c_execute(plan: int, stream, d_timeseries, d_spectrum, scale: float = 1.0) -> None:
-    _check(lib.fdas_r2c_execute(plan, _stream(stream), _ptr(d_timeseries), _ptr(d_spectrum), float(scale)),
-           "fdas_r2c_execute")
+    st = lib.fdas_r2c_execute(plan, _stream(stream), _ptr(d_timeseries), _ptr(d_spectrum), float(scale))
+    if st != FDAS_OK:
+        raise FdasError(st, "fdas_r2c_execute", lib.fdas_last_error(None).decode() if st == 5 else "")
 
 
 def fdas_r2c_destroy(plan: int) -> None:

@@ -34,6 +34,13 @@ More pins: `dft_real*` by a literal O(n^2) Python loop, a pure tone's bin and am
 symmetry, linearity, the shift theorem and numpy's rfft as a third opinion; `harmonic_sum` by literal loops on a
 tiny plane, the identity at one harmonic, a time-domain signal with power in harmonics 1, 2 and 4 peaking at the
 fundamental's cell, and the Erlang tail law of summed noise powers.
+  * the two steps between that transform and the correlations (Fig. 2): red-noise removal by a local
+    median filter, `deredden`, and the normalisation of each block, `normalise_blocks` (readings R19, R20).
+
+Pins of those two (tests/test_oracle_pins_whiten.py, P15): a hand-sorted tiny input, the exponential law's
+median = mean x ln 2 (white noise keeps unit mean power), a power-law spectrum coming out flat, a strong narrow tone
+surviving within 1/block of its amplitude, block mean exactly 1 after normalisation, scale invariance / idempotence,
+the ragged last block and the all-zero block.
 No function here is "parity unpinned".
 """
 from __future__ import annotations
@@ -362,3 +369,44 @@ def harmonic_candidates(plane: np.ndarray, zmax: float, dz: float, nharm: int, t
     rows = harmonic_rows(zmax, dz, nharm)
     i, c = np.nonzero(s > threshold)
     return rows[i].astype(np.int64), c.astype(np.int64), s[i, c]
+
+
+# --------------------------------------------------------------------------------------
+# red-noise removal and block normalisation (Fig. 2; readings R19, R20)
+# --------------------------------------------------------------------------------------
+
+
+def _scale_blocks(spectrum: np.ndarray, block: int, statistic) -> np.ndarray:
+    """out[j] = A[j] / sqrt(statistic(powers of A's block)): consecutive blocks of `block` bins from bin 0, the last
+    one shorter when `block` does not divide N; a block whose statistic is 0 is copied unchanged."""
+    a = np.asarray(spectrum).astype(np.complex128).reshape(-1)
+    block = int(block)
+    if block < 1:
+        raise ValueError("block must be >= 1")
+    out = a.copy()
+    for start in range(0, a.size, block):
+        seg = a[start:start + block]
+        stat = float(statistic(seg.real ** 2 + seg.imag ** 2))
+        if stat > 0.0:
+            out[start:start + block] = seg / math.sqrt(stat)
+    return out
+
+
+def deredden(spectrum: np.ndarray, block: int) -> np.ndarray:
+    """
+    "low frequency (red) noise is removed with the use of a local median filter".  Reading R19: the
+    local noise level of a block of `block` consecutive bins is estimated by the MEDIAN of its Fourier powers
+    |A[j]|^2 (the median ignores the few bins a signal occupies); noise powers are exponentially distributed, whose
+    median is mean x ln 2, so the block is divided by sqrt(median / ln 2) and its noise comes out at unit mean power.
+    Median of an even count = mean of the two middle values.  fp64, complex128 out.
+    """
+    return _scale_blocks(spectrum, block, lambda p: np.median(p) / math.log(2.0))
+
+
+def normalise_blocks(spectrum: np.ndarray, block: int) -> np.ndarray:
+    """
+    "After a short step of normalization on the data of each block, the matched filtering is performed"
+    (PAPER.md:79).  Reading R20: the blocks are the overlap-save blocks (`block` = the useful bins B of a segment)
+    and each is scaled to unit MEAN power, A[j] / sqrt(mean_j |A[j]|^2).  fp64, complex128 out.
+    """
+    return _scale_blocks(spectrum, block, np.mean)

@@ -254,6 +254,31 @@ fdas_status fdas_r2c_destroy(fdas_r2c_plan *plan);
 fdas_status fdas_r2c_execute_static(void *stream, const float *d_timeseries, int64_t nsamples, void *d_spectrum,
                                     float scale);
 
+/* ---- red-noise removal and block normalisation between the transform and the correlations (8(f) F3) ---- */
+
+typedef enum { FDAS_WHITEN_MEDIAN = 0, FDAS_WHITEN_MEAN = 1 } fdas_whiten_statistic;
+
+/*
+ * Scale every block of `block` consecutive bins of a spectrum by one positive real number taken from the block's own
+ * Fourier powers (Fig. 2; the paper names the two steps without formulas -- DESIGN.md readings R19, R20):
+ *     out[j] = A[j] / sqrt(stat_b),  b = j / block  (blocks start at bin 0; the last one may be shorter)
+ *   FDAS_WHITEN_MEDIAN  stat_b = median |A|^2 / ln 2 : "low frequency (red) noise is removed with the use of a local
+ *                       median filter" -- the median is blind to the few bins a signal occupies, and exponentially
+ *                       distributed noise powers have median = mean x ln 2, so the noise comes out at unit mean power.
+ *                       The median is exact (mean of the two middle values for an even count).
+ *   FDAS_WHITEN_MEAN    stat_b = mean |A|^2 : "a short step of normalization on the data of each block" -- call it
+ *                       with block = fdas_info.useful so that blocks are the plan's overlap-save blocks.
+ * A block whose statistic is 0 is copied unchanged.  Inputs are assumed finite with |A|^2 below the float32 range.
+ *   d_spectrum : device, nbins x {float re, float im}, 8-byte aligned; read only (twice).
+ *   d_out      : device, same shape; may be d_spectrum itself (in place); must not overlap it otherwise.
+ * One launch on `stream` (one CTA per block), no plan, no allocation, no host synchronisation; chains between
+ * fdas_r2c_execute and fdas_execute on one stream.
+ * Errors: FDAS_ERR_INVALID_ARG (null pointers, nbins <= 0, unknown statistic), FDAS_ERR_UNSUPPORTED (block outside
+ * [32, 8192]; text in fdas_last_error(NULL)), FDAS_ERR_ALIGNMENT, FDAS_ERR_CUDA.
+ */
+fdas_status fdas_whiten(void *stream, const void *d_spectrum, void *d_out, int64_t nbins, int32_t block,
+                        int32_t statistic);
+
 /* ---- introspection for harnesses and tests (not on the hot path) ---- */
 
 fdas_status fdas_plan_info(const fdas_plan *plan, fdas_info *out);
@@ -285,7 +310,7 @@ int64_t fdas_launch_count(void);
 
 const char *fdas_status_string(fdas_status s);
 /* Text of the last CUDA error seen by this plan ("" if none); plan = NULL: of the calling thread's last
- * failed fdas_plan_create, fdas_r2c_plan_create, fdas_r2c_execute or fdas_r2c_execute_static. */
+ * failed fdas_plan_create, fdas_r2c_plan_create, fdas_r2c_execute, fdas_r2c_execute_static or fdas_whiten. */
 const char *fdas_last_error(const fdas_plan *plan);
 
 #ifdef __cplusplus

@@ -8,7 +8,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfdas.so")
 SOURCES = [os.path.join(CSRC, "fdas_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fdas_fft.cuh", "fdas_kernel.cuh", "fdas_kernel8k.cuh", "fdas_kernel2.cuh", "fdas_kernel3.cuh", "fdas_r2c.cuh", "fdas_templates.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fdas_fft.cuh", "fdas_kernel.cuh", "fdas_kernel8k.cuh", "fdas_kernel2.cuh", "fdas_kernel3.cuh", "fdas_r2c.cuh", "fdas_whiten.cuh", "fdas_templates.cuh")] + [
     os.path.join(ROOT, "include", "fdas.h")]
 
 

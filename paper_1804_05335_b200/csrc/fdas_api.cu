@@ -715,6 +715,30 @@ fdas_status fdas_r2c_destroy(fdas_r2c_plan *p)
     return FDAS_OK;
 }
 
+// ---------------------------------------------------------------- red-noise removal / block normalisation (fdas_whiten.cuh)
+fdas_status fdas_whiten(void *stream, const void *d_spectrum, void *d_out, int64_t nbins, int32_t block,
+                        int32_t statistic)
+{
+    if (!d_spectrum || !d_out || nbins <= 0 || (statistic != FDAS_WHITEN_MEDIAN && statistic != FDAS_WHITEN_MEAN))
+        return FDAS_ERR_INVALID_ARG;
+    const long long nblocks = block > 0 ? (nbins + block - 1) / block : 0;
+    if (block < WHITEN_MIN_BLOCK || block > WHITEN_MAX_BLOCK || nblocks > 0x7fffffffll) {
+        snprintf(g_create_err, sizeof(g_create_err), "fdas_whiten: block = %d, nbins = %lld; needs %d <= block <= %d and at "
+                 "most 2^31 - 1 blocks", (int)block, (long long)nbins, WHITEN_MIN_BLOCK, WHITEN_MAX_BLOCK);
+        return FDAS_ERR_UNSUPPORTED;
+    }
+    if (((uintptr_t)d_spectrum & 7) || ((uintptr_t)d_out & 7)) return FDAS_ERR_ALIGNMENT;
+    whiten_kernel<<<(unsigned)nblocks, WHITEN_THREADS, whiten_smem_bytes(block), (cudaStream_t)stream>>>(
+        (const float2 *)d_spectrum, (float2 *)d_out, nbins, block, statistic);
+    g_launches += 1;
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        snprintf(g_create_err, sizeof(g_create_err), "fdas_whiten: %s", cudaGetErrorString(e));
+        return FDAS_ERR_CUDA;
+    }
+    return FDAS_OK;
+}
+
 // ---------------------------------------------------------------- the transform for callers that may not allocate
 } // extern "C"
 

@@ -17,6 +17,7 @@
 #include "fdas_kernel2.cuh"
 #include "fdas_kernel3.cuh"
 #include "fdas_r2c.cuh"
+#include "fdas_whiten.cuh"
 
 namespace fdas {
 

@@ -24,7 +24,9 @@ EXPORTS = ["fdas_plan_create", "fdas_make_templates", "fdas_execute", "fdas_exec
            "fdas_plan_info", "fdas_get_taps", "fdas_get_template_spectrum", "fdas_measure_fp32_peak",
            "fdas_launch_count", "fdas_status_string", "fdas_last_error",
            "fdas_harmonic_sum_threshold", "fdas_r2c_plan_create", "fdas_r2c_execute", "fdas_r2c_destroy",
-           "fdas_r2c_execute_static"]
+           "fdas_r2c_execute_static", "fdas_whiten"]
+
+WHITEN_MEDIAN, WHITEN_MEAN = 0, 1     # fdas_whiten_statistic
 
 R2C_STATIC_MAX_SAMPLES = 1 << 20      # FDAS_R2C_STATIC_MAX_SAMPLES of include/fdas.h
 
@@ -68,6 +70,7 @@ def _load() -> ctypes.CDLL:
     lib.fdas_r2c_execute.argtypes = [vp, vp, vp, vp, ctypes.c_float]
     lib.fdas_r2c_destroy.argtypes = [vp]
     lib.fdas_r2c_execute_static.argtypes = [vp, vp, i64, vp, ctypes.c_float]
+    lib.fdas_whiten.argtypes = [vp, vp, vp, i64, i32, i32]
     lib.fdas_plan_info.argtypes = [vp, ctypes.POINTER(FdasInfo)]
     lib.fdas_get_taps.argtypes = [vp, i32, vp, ctypes.POINTER(i32)]
     lib.fdas_get_template_spectrum.argtypes = [vp, i32, vp]
@@ -181,6 +184,12 @@ def fdas_r2c_execute_static(stream, d_timeseries, nsamples: int, d_spectrum, sca
     st = lib.fdas_r2c_execute_static(_stream(stream), _ptr(d_timeseries), int(nsamples), _ptr(d_spectrum), float(scale))
     if st != FDAS_OK:
         raise FdasError(st, "fdas_r2c_execute_static", lib.fdas_last_error(None).decode() if st in (2, 5) else "")
+
+
+def fdas_whiten(stream, d_spectrum, d_out, nbins: int, block: int, statistic: int) -> None:
+    st = lib.fdas_whiten(_stream(stream), _ptr(d_spectrum), _ptr(d_out), int(nbins), int(block), int(statistic))
+    if st != FDAS_OK:
+        raise FdasError(st, "fdas_whiten", lib.fdas_last_error(None).decode() if st in (2, 5) else "")
 
 
 def fdas_destroy(plan: int) -> None:

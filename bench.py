@@ -418,6 +418,28 @@ def time_r2c(torch, fdas, dev, stream, n, peaks, steps=20):
                   % (16 * n >> 20, "stays in" if 16 * n < (120 << 20) else "larger than")}
 
 
+def time_whiten(torch, fdas, dev, stream, n, block, statistic, peaks, steps=20):
+    """fdas_whiten on n bins (red-noise removal by a local median filter / per-block normalisation):
+    one launch, HBM-bound: 8n bytes read + 8n written.  Inputs rotate over > 126 MB so no call finds its input in L2."""
+    nin = max(2, (160 << 20) // (8 * n) + 1)
+    xs = torch.randn((nin, n, 2), dtype=torch.float32, device=dev)
+    out = torch.empty((n, 2), dtype=torch.float32, device=dev)
+    with torch.cuda.stream(stream):
+        for i in range(3):
+            fdas.fdas_whiten(stream, xs[i % nin], out, n, block, statistic)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for i in range(steps):
+            fdas.fdas_whiten(stream, xs[i % nin], out, n, block, statistic)
+        e1.record(stream)
+    stream.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    gbs = 16.0 * n / (ms * 1e-3) / 1e9
+    return {"nbins": n, "block": block, "statistic": "median" if statistic == 0 else "mean", "ms": ms,
+            "bins_per_s": n / (ms * 1e-3), "alg_bytes": 16 * n, "achieved_gbs": gbs, "frac_hbm": gbs / peaks["hbm_gbs"],
+            "launches_per_call": 1}
+
+
 def time_harmonics(torch, fdas, synthetic, dev, stream, w, peaks):
     """fdas_harmonic_sum_threshold over a stored plane of config `w` for H = 2, 4, 8, 16."""
     import numpy as np
@@ -682,6 +704,9 @@ def main():
     if rank == 0 and world == 1 and not args.no_configs:
         try:
             extra["r2c"] = {str(n): time_r2c(torch, fdas, dev, stream, n, peaks) for n in (1 << 21, 1 << 23, 1 << 24)}
+            extra["whiten"] = [time_whiten(torch, fdas, dev, stream, n, b, st_, peaks)
+                               for (n, b, st_) in ((1 << 21, 1024, 0), (1 << 21, 1920, 1), (1 << 23, 1024, 0),
+                                                   (1 << 23, 4096, 0), (1 << 23, 7936, 1))]
             extra["harmonic_sum"] = time_harmonics(torch, fdas, synthetic, dev, stream, workload(2), peaks)
         except Exception as exc:                      # the next-row extras must not cost the bench line
             extra["extras_unavailable"] = f"{type(exc).__name__}: {exc}"[:200]

@@ -33,7 +33,8 @@ twice its length, a half-bin tone's full recovery and the time-domain chirp at a
 More pins: `dft_real*` by a literal O(n^2) Python loop, a pure tone's bin and amplitude, Parseval, conjugate
 symmetry, linearity, the shift theorem and numpy's rfft as a third opinion; `harmonic_sum` by literal loops on a
 tiny plane, the identity at one harmonic, a time-domain signal with power in harmonics 1, 2 and 4 peaking at the
-fundamental's cell, and the Erlang tail law of summed noise powers.
+fundamental's cell, and the Erlang tail law of summed noise powers; `harmonic_sums_cumulative` (one walk over the
+harmonics for H = 2, 4, 8, 16) by equality with `harmonic_sum` level by level and a hand-computed cell.
   * the two steps between that transform and the correlations (Fig. 2): red-noise removal by a local
     median filter, `deredden`, and the normalisation of each block, `normalise_blocks` (readings R19, R20).
 
@@ -369,6 +370,37 @@ def harmonic_candidates(plane: np.ndarray, zmax: float, dz: float, nharm: int, t
     rows = harmonic_rows(zmax, dz, nharm)
     i, c = np.nonzero(s > threshold)
     return rows[i].astype(np.int64), c.astype(np.int64), s[i, c]
+
+
+def harmonic_sums_cumulative(plane: np.ndarray, zmax: float, dz: float, levels=(2, 4, 8, 16)) -> dict:
+    """
+    The sums S_H of `harmonic_sum` for an increasing list of H, formed the way a search does it in ONE walk over the
+    harmonics of a fundamental cell ("adding the power that is distributed in the harmonics to that of
+    the fundamental"; reading R18):  S_{H_l}[k][c] = S_{H_{l-1}}[k][c] + sum_{h = H_{l-1}+1}^{H_l} P[row(h z_k)][h c],
+    S_{H_0 = 0} = 0, on the rows and columns of level l (|z_k| <= zmax / H_l, H_l c <= ncols - 1), which shrink with l.
+    Returns {H: (rows, S_H)} with S_H as `harmonic_sum` shapes it.  A literal loop over cells; small planes only.
+    """
+    p = np.asarray(plane, dtype=np.float64)
+    k_all, ncols = p.shape
+    nhalf = (k_all - 1) // 2
+    levels = [int(h) for h in levels]
+    if any(b <= a for a, b in zip([0] + levels, levels)):
+        raise ValueError("levels must be increasing and positive")
+    out = {h: (harmonic_rows(zmax, dz, h), np.zeros((harmonic_rows(zmax, dz, h).size, (ncols - 1) // h + 1)))
+           for h in levels}
+    rows0 = harmonic_rows(zmax, dz, levels[0])
+    for k in rows0:
+        for c in range((ncols - 1) // levels[0] + 1):
+            s, h_done = 0.0, 0
+            for hl in levels:
+                lim = nhalf // hl
+                if abs(int(k) - nhalf) > lim or hl * c > ncols - 1:
+                    break                                     # this cell is outside level hl and every later one
+                for h in range(h_done + 1, hl + 1):
+                    s += p[nhalf + h * (int(k) - nhalf), h * c]
+                h_done = hl
+                out[hl][1][int(k) - (nhalf - lim), c] = s
+    return out
 
 
 # --------------------------------------------------------------------------------------

@@ -11,6 +11,7 @@ import os
 import sys
 
 import numpy as np
+import pytest
 
 sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
 
@@ -146,3 +147,28 @@ def test_p14_noise_mean_and_erlang_tail():
         tail = math.exp(-t) * sum(t ** j / math.factorial(j) for j in range(H))
         frac = np.count_nonzero(s > t) / s.size
         assert abs(frac - tail) < 5.0 * math.sqrt(tail / s.size) + 1e-6
+
+
+def test_cumulative_harmonic_sums_equal_the_per_h_definition():
+    """P14 extended: the one-walk form (S_4 = S_2 + P[3z][3c] + P[4z][4c], ...) is the same function as the per-H
+    definition on every level's own domain; one cell by hand."""
+    rng = np.random.Generator(np.random.Philox(99))
+    zmax, dz = 32.0, 2.0
+    plane = rng.standard_exponential((33, 203))
+    cum = orc.harmonic_sums_cumulative(plane, zmax, dz, (2, 4, 8, 16))
+    for hh in (2, 4, 8, 16):
+        rows, s = cum[hh]
+        assert np.array_equal(rows, orc.harmonic_rows(zmax, dz, hh))
+        ref = orc.harmonic_sum(plane, zmax, dz, hh)
+        assert s.shape == ref.shape and np.max(np.abs(s - ref)) <= 1e-12 * ref.max()
+    # by hand: fundamental z = +2 (row 17 of 33), column 5: S_4 collects rows 17, 18, 19, 20 at columns 5, 10, 15, 20
+    want = plane[17, 5] + plane[18, 10] + plane[19, 15] + plane[20, 20]
+    rows, s4 = cum[4]
+    assert abs(s4[list(rows).index(17), 5] - want) <= 1e-14 * want
+    # other level lists: a single level is harmonic_sum itself; a level the bank cannot hold keeps only z = 0
+    one = orc.harmonic_sums_cumulative(plane, zmax, dz, (3,))
+    assert np.allclose(one[3][1], orc.harmonic_sum(plane, zmax, dz, 3), rtol=1e-13)
+    big = orc.harmonic_sums_cumulative(plane, zmax, dz, (2, 32))
+    assert big[32][0].tolist() == [16] and big[32][1].shape == (1, (203 - 1) // 32 + 1)
+    with pytest.raises(ValueError):
+        orc.harmonic_sums_cumulative(plane, zmax, dz, (4, 2))

@@ -181,6 +181,25 @@ fdas_status fdas_harmonic_sum_threshold(fdas_plan *plan, void *stream, const flo
                                         float threshold, fdas_candidate *d_cands, int64_t capacity,
                                         uint64_t *d_count);
 
+/*
+ * The harmonic search for several H in one pass ("adding the power that is distributed in the harmonics to
+ * that of the fundamental", :331; reading R18): for the increasing list nharm[0..nlevels) (usually 2, 4, 8, 16) the sums
+ * are formed cumulatively while walking the harmonics of each fundamental cell once,
+ *     S_{H_l}[k][c] = S_{H_{l-1}}[k][c] + sum_{h = H_{l-1}+1}^{H_l} P[row(h z_k)][h c],
+ * and level l's cells with S_{H_l} > thresholds[l] go to level l's own list.  Each level's candidates are exactly
+ * (same cells, same float32 sums bit for bit) those of fdas_harmonic_sum_threshold(nharm[l], thresholds[l]); the
+ * fundamental rows are read once instead of once per H.  One launch on `stream`, no allocation, no host sync.
+ *   nharm, thresholds : HOST arrays of nlevels entries, 1 <= nlevels <= 4, nharm strictly increasing, >= 1.
+ *   d_cands  : device, nlevels x capacity fdas_candidate, 16-byte aligned; level l's list starts at l * capacity
+ *              (not checked when capacity is 0).
+ *   d_counts : device, nlevels x uint64, zeroed on `stream` first; counts[l] may exceed capacity (then only the
+ *              first `capacity` candidates of that level were stored).  Order within a list is unspecified.
+ * Errors: as fdas_harmonic_sum_threshold, plus FDAS_ERR_INVALID_ARG for a bad level list.
+ */
+fdas_status fdas_harmonic_sums_threshold(fdas_plan *plan, void *stream, const float *d_plane, int32_t nlevels,
+                                         const int32_t *nharm, const float *thresholds, fdas_candidate *d_cands,
+                                         int64_t capacity, uint64_t *d_counts);
+
 /* Free the plan and everything it owns.  fdas_destroy(NULL) is a no-op returning FDAS_OK. */
 fdas_status fdas_destroy(fdas_plan *plan);
 

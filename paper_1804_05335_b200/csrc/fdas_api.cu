@@ -511,6 +511,43 @@ fdas_status fdas_harmonic_sum_threshold(fdas_plan *p, void *stream, const float 
     return FDAS_OK;
 }
 
+fdas_status fdas_harmonic_sums_threshold(fdas_plan *p, void *stream, const float *d_plane, int32_t nlevels,
+                                         const int32_t *nharm, const float *thresholds, fdas_candidate *d_cands,
+                                         int64_t capacity, uint64_t *d_counts)
+{
+    if (!p || !d_plane || !d_counts || !nharm || !thresholds || nlevels < 1 || nlevels > 4 || capacity < 0 ||
+        (capacity > 0 && !d_cands) || !on_plan_device(p))
+        return FDAS_ERR_INVALID_ARG;
+    HarmonicLevels lv;
+    std::memset(&lv, 0, sizeof(lv));
+    for (int l = 0; l < nlevels; ++l) {
+        if (nharm[l] < 1 || (l > 0 && nharm[l] <= nharm[l - 1]) || thresholds[l] != thresholds[l])
+            return FDAS_ERR_INVALID_ARG;
+        lv.nharm[l] = nharm[l];
+        lv.threshold[l] = thresholds[l];
+    }
+    if (((uintptr_t)d_plane & 15) || (capacity > 0 && ((uintptr_t)d_cands & 15)) || ((uintptr_t)d_counts & 7))
+        return FDAS_ERR_ALIGNMENT;
+    const fdas_info &I = p->info;
+    cudaStream_t st = (cudaStream_t)stream;
+    FDAS_CUDA(p, cudaMemsetAsync(d_counts, 0, sizeof(uint64_t) * nlevels, st));
+    lv.nlevels = nlevels;
+    lv.capacity = capacity;
+    lv.cands = (Candidate *)d_cands;
+    lv.counts = (unsigned long long *)d_counts;
+    const int nhalf = (I.ntemplates - 1) / 2, lim = nhalf / nharm[0];       // the first level has the widest domain
+    const long long nc = (I.ncols - 1) / nharm[0] + 1;
+    const long long nbx = (nc + 1023) / 1024, nblocks = nbx * (2 * lim + 1);
+    if (nblocks > 0x7fffffffll) {
+        snprintf(p->err, sizeof(p->err), "fdas_harmonic_sums_threshold: %lld CTAs exceed the grid limit", nblocks);
+        return FDAS_ERR_UNSUPPORTED;
+    }
+    harmonic_sums_kernel<<<(unsigned)nblocks, 256, 0, st>>>(d_plane, I.ncols, I.ntemplates, (unsigned)nbx, lv);
+    g_launches += 1;
+    FDAS_CUDA(p, cudaGetLastError());
+    return FDAS_OK;
+}
+
 fdas_status fdas_destroy(fdas_plan *p)
 {
     if (!p) return FDAS_OK;

@@ -246,4 +246,60 @@ __global__ void __launch_bounds__(256) harmonic_sum_kernel(const float *__restri
     }
 }
 
+// Harmonic sums for several H in ONE walk over the harmonics of a fundamental cell (fdas_harmonic_sums_threshold,
+// include/fdas.h; reading R18): S_{H_l} = S_{H_{l-1}} + sum_{h = H_{l-1}+1}^{H_l} P[row(h z_k)][h c],
+// compared with level l's threshold as soon as it is complete and appended to level l's own list.  The grid covers the
+// rows and columns of the first level; a cell leaves the walk at the first level whose domain (|z_k| <= zmax / H_l,
+// H_l c <= ncols - 1) it is outside -- for a whole CTA when its row or its column block is (uniform branch).  The
+// additions run in the order h = 1, 2, .. like harmonic_sum_kernel's, so each level's sums are bit-identical to a
+// separate launch of that kernel; the fundamental rows are read once instead of once per H.
+struct HarmonicLevels {
+    int nlevels;
+    int nharm[4];
+    float threshold[4];
+    long long capacity;          // per level
+    Candidate *cands;            // nlevels x capacity
+    unsigned long long *counts;  // nlevels
+};
+
+__global__ void __launch_bounds__(256) harmonic_sums_kernel(const float *__restrict__ plane, long long ncols, int K,
+                                                            unsigned nbx, const HarmonicLevels lv)
+{
+    const unsigned by = blockIdx.x / nbx, bx = blockIdx.x - by * nbx;
+    const int center = (K - 1) / 2;
+    const int dk = (int)by - center / lv.nharm[0];                 // row offset from z = 0 of this CTA's fundamental
+    const long long cb = (long long)bx * (4 * blockDim.x), c0 = cb + threadIdx.x;
+    float s[4] = {0.f, 0.f, 0.f, 0.f};
+    int h = 1;
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {                                  // unrolled: lv stays in the parameter bank
+        if (l >= lv.nlevels) return;
+        const int hl = lv.nharm[l];
+        const long long nc = (ncols - 1) / hl + 1;
+        if ((dk < 0 ? -dk : dk) > center / hl || cb >= nc) return;
+        for (; h <= hl; ++h) {
+            const float *row = plane + (size_t)(center + h * dk) * ncols;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const long long c = c0 + (long long)j * blockDim.x;
+                if (c < nc) s[j] += __ldg(row + h * c);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const long long c = c0 + (long long)j * blockDim.x;
+            if (c < nc && s[j] > lv.threshold[l]) {
+                const unsigned long long slot = atomicAdd(lv.counts + l, 1ull);
+                if (slot < (unsigned long long)lv.capacity) {
+                    Candidate cd;
+                    cd.col = c;
+                    cd.row = center + dk;
+                    cd.power = s[j];
+                    lv.cands[(size_t)l * lv.capacity + slot] = cd;
+                }
+            }
+        }
+    }
+}
+
 } // namespace fdas

@@ -24,7 +24,8 @@ EXPORTS = ["fdas_plan_create", "fdas_make_templates", "fdas_execute", "fdas_exec
            "fdas_plan_info", "fdas_get_taps", "fdas_get_template_spectrum", "fdas_measure_fp32_peak",
            "fdas_launch_count", "fdas_status_string", "fdas_last_error",
            "fdas_harmonic_sum_threshold", "fdas_r2c_plan_create", "fdas_r2c_execute", "fdas_r2c_destroy",
-           "fdas_r2c_execute_static", "fdas_whiten"]
+           "fdas_r2c_execute_static", "fdas_whiten",
+           "fdas_harmonic_sums_threshold"]
 
 WHITEN_MEDIAN, WHITEN_MEAN = 0, 1     # fdas_whiten_statistic
 
@@ -71,6 +72,8 @@ def _load() -> ctypes.CDLL:
     lib.fdas_r2c_destroy.argtypes = [vp]
     lib.fdas_r2c_execute_static.argtypes = [vp, vp, i64, vp, ctypes.c_float]
     lib.fdas_whiten.argtypes = [vp, vp, vp, i64, i32, i32]
+    lib.fdas_harmonic_sums_threshold.argtypes = [vp, vp, vp, i32, ctypes.POINTER(i32), ctypes.POINTER(ctypes.c_float), vp,
+                                                 i64, vp]
     lib.fdas_plan_info.argtypes = [vp, ctypes.POINTER(FdasInfo)]
     lib.fdas_get_taps.argtypes = [vp, i32, vp, ctypes.POINTER(i32)]
     lib.fdas_get_template_spectrum.argtypes = [vp, i32, vp]
@@ -157,6 +160,14 @@ def fdas_harmonic_sum_threshold(plan: int, stream, d_plane, nharm: int, threshol
     _check(lib.fdas_harmonic_sum_threshold(plan, _stream(stream), _ptr(d_plane), int(nharm), float(threshold),
                                            _ptr(d_cands), int(capacity), _ptr(d_count)),
            "fdas_harmonic_sum_threshold", plan)
+
+
+def fdas_harmonic_sums_threshold(plan: int, stream, d_plane, nharm, thresholds, d_cands, capacity: int, d_counts) -> None:
+    n = len(nharm)
+    assert len(thresholds) == n
+    _check(lib.fdas_harmonic_sums_threshold(plan, _stream(stream), _ptr(d_plane), n, (ctypes.c_int32 * n)(*map(int, nharm)),
+                                            (ctypes.c_float * n)(*map(float, thresholds)), _ptr(d_cands), int(capacity),
+                                            _ptr(d_counts)), "fdas_harmonic_sums_threshold", plan)
 
 
 def fdas_r2c_plan_create(nsamples: int) -> int:
@@ -259,6 +270,9 @@ class Plan:
 
     def harmonic_sum_threshold(self, stream, d_plane, nharm, threshold, d_cands, capacity, d_count):
         fdas_harmonic_sum_threshold(self.handle, stream, d_plane, nharm, threshold, d_cands, capacity, d_count)
+
+    def harmonic_sums_threshold(self, stream, d_plane, nharm, thresholds, d_cands, capacity, d_counts):
+        fdas_harmonic_sums_threshold(self.handle, stream, d_plane, nharm, thresholds, d_cands, capacity, d_counts)
 
     def execute_host(self, stream, h_spectrum, h_plane):
         fdas_execute_host(self.handle, stream, h_spectrum, h_plane)

@@ -267,3 +267,131 @@ def test_harmonic_sum_bank_of_more_than_65535_rows(torch, fd, orc, nharm):
     index_of = {int(r): i for i, r in enumerate(rows)}
     for (rr, c_) in set(zip(r_o.tolist(), c_o.tolist())) ^ set(zip(got["row"].tolist(), got["col"].tolist())):
         assert near[index_of[rr], c_], (rr, c_)
+
+
+# ---------------------------------------------------------------- harmonic sums for several H in one pass
+def read_level(torch, d_cands, d_counts, cap, level):
+    cnt = int(d_counts[level].item())
+    assert cnt <= cap
+    rec = d_cands[level * cap * 16:(level * cap + cnt) * 16].cpu().numpy().copy().view(
+        [("col", "<i8"), ("row", "<i4"), ("power", "<f4")])
+    return rec[np.lexsort((rec["col"], rec["row"]))]
+
+
+@pytest.mark.parametrize("levels", [(2, 4, 8, 16), (1, 2, 3), (4,), (2, 32)])
+@pytest.mark.parametrize("interbin", [0, 1])
+def test_one_pass_harmonic_sums_match_per_h_calls_and_oracle(torch, fd, orc, levels, interbin):
+    """fdas_harmonic_sums_threshold: each level's list equals fdas_harmonic_sum_threshold's for that H bit for bit, and
+    the sums agree with the oracle's cumulative walk (oracle.harmonic_sums_cumulative) over the same stored plane."""
+    from paper_1804_05335_b200 import synthetic as syn
+    n, zmax, dz = 9000, 32.0, 2.0
+    r0, z0 = 400.0, 2.0
+    chirps = [(h * r0, h * z0, a) for h, a in ((1, 6.0), (2, 5.0), (4, 4.0), (8, 3.5), (16, 3.0))]
+    spec = syn.make_spectrum(n, 78, chirps)
+    with fd.Plan(n, zmax, dz, 1024, interbin) as plan:
+        plan.make_templates()
+        K, ncols = plan.info.ntemplates, plan.info.ncols
+        st = torch.cuda.current_stream()
+        d_spec = torch.from_numpy(spec.view(np.float32).reshape(n, 2)).cuda()
+        d_plane = torch.empty((K, ncols), dtype=torch.float32, device="cuda")
+        plan.execute(st, d_spec, d_plane)
+        cap = 1 << 16
+        nl = len(levels)
+        thr = [h + 3.0 * math.sqrt(h) + 3.0 for h in levels]
+        d_cands = torch.zeros(nl * cap * 16, dtype=torch.uint8, device="cuda")
+        d_counts = torch.full((nl,), 123, dtype=torch.int64, device="cuda")
+        launches0 = fd.fdas_launch_count()
+        plan.harmonic_sums_threshold(st, d_plane, levels, thr, d_cands, cap, d_counts)
+        assert fd.fdas_launch_count() - launches0 == 1
+        torch.cuda.synchronize()
+        multi = [read_level(torch, d_cands, d_counts, cap, l) for l in range(nl)]
+        d_c1 = torch.zeros(cap * 16, dtype=torch.uint8, device="cuda")
+        d_n1 = torch.zeros(1, dtype=torch.int64, device="cuda")
+        for l, h in enumerate(levels):
+            plan.harmonic_sum_threshold(st, d_plane, h, thr[l], d_c1, cap, d_n1)
+            torch.cuda.synchronize()
+            single = read_cands(torch, d_c1, d_n1, cap)
+            assert multi[l].size == single.size and multi[l].tobytes() == single.tobytes(), (l, h)
+        plane = d_plane.cpu().numpy()
+    assert multi[0].size > 0
+    cum = orc.harmonic_sums_cumulative(plane, zmax, dz, levels)         # fp64 walk over the stored float32 cells
+    for l, h in enumerate(levels):
+        rows, s64 = cum[h]
+        index_of = {int(r): i for i, r in enumerate(rows)}
+        got = multi[l]
+        ref = np.array([s64[index_of[int(r)], int(c)] for r, c in zip(got["row"], got["col"])])
+        assert np.all(np.abs(got["power"] - ref) <= 2e-6 * np.maximum(ref, 1.0))
+        ii, cc = np.nonzero(s64 > thr[l])
+        near = np.abs(s64 - thr[l]) < 1e-5 * thr[l]
+        for (rr, c_) in set(zip(rows[ii].tolist(), cc.tolist())) ^ set(zip(got["row"].tolist(), got["col"].tolist())):
+            assert near[index_of[rr], c_], (h, rr, c_)
+
+
+def test_one_pass_harmonic_sums_config2_full_size(torch, fd, orc):
+    """BASELINE config 2 at its stated size (85 x 2^21 plane from fdas_execute): the one-pass search for H = 2, 4, 8, 16
+    against (a) float32 sums of the stored plane in the kernel's order, every level, every cell -- exact; (b) the
+    oracle's fp64 sums of the ORACLE'S OWN plane rows on sampled fundamentals (z = 6 at H = 2, z = 2 at H = 4, z = 0 at
+    H = 8 and 16), as the config-5 parity test samples."""
+    from paper_1804_05335_b200 import synthetic as syn
+    c = syn.CONFIGS[1]
+    n, zmax, dz = c["nbins"], c["zmax"], c["dz"]
+    assert (n, c["seglen"]) == (1 << 21, 2048)
+    spec, _ = syn.config_spectrum(1, 0)
+    levels, thr = (2, 4, 8, 16), [13.0, 18.0, 24.0, 36.0]
+    with fd.Plan(n, zmax, dz, c["seglen"], 0) as plan:
+        plan.make_templates()
+        K, ncols = plan.info.ntemplates, plan.info.ncols
+        st = torch.cuda.current_stream()
+        d_spec = torch.from_numpy(spec.view(np.float32).reshape(n, 2)).cuda()
+        d_plane = torch.empty((K, ncols), dtype=torch.float32, device="cuda")
+        plan.execute(st, d_spec, d_plane)
+        cap = 1 << 20
+        d_cands = torch.zeros(4 * cap * 16, dtype=torch.uint8, device="cuda")
+        d_counts = torch.zeros(4, dtype=torch.int64, device="cuda")
+        plan.harmonic_sums_threshold(st, d_plane, levels, thr, d_cands, cap, d_counts)
+        torch.cuda.synchronize()
+        multi = [read_level(torch, d_cands, d_counts, cap, l) for l in range(4)]
+        plane = d_plane.cpu().numpy()
+    nhalf = (K - 1) // 2
+    zs = orc.bank_z(zmax, dz)
+    for l, h in enumerate(levels):
+        rows = orc.harmonic_rows(zmax, dz, h)
+        nc = (ncols - 1) // h + 1
+        s32 = np.zeros((rows.size, nc), dtype=np.float32)
+        for hh in range(1, h + 1):
+            s32 += plane[nhalf + hh * (rows - nhalf)][:, 0:hh * (nc - 1) + 1:hh]
+        ii, cc = np.nonzero(s32 > np.float32(thr[l]))
+        got = multi[l]
+        assert got.size == ii.size > 0, (h, got.size, ii.size)
+        assert np.array_equal(got["row"], rows[ii]) and np.array_equal(got["col"], cc)
+        assert np.array_equal(got["power"], s32[ii, cc])
+        # (b) the oracle's own plane rows for one fundamental per level
+        zf = {2: 6.0, 4: 2.0, 8: 0.0, 16: 0.0}[h]
+        kf = int(np.nonzero(zs == zf)[0][0])
+        s_or = np.zeros(nc)
+        for hh in range(1, h + 1):
+            s_or += orc.plane_row(spec, hh * zf, False)[0:hh * (nc - 1) + 1:hh]
+        i_f = int(np.nonzero(rows == kf)[0][0])
+        assert np.max(np.abs(s32[i_f] - s_or)) <= 1e-4 * s_or.max()
+        want = set(np.nonzero(s_or > thr[l])[0].tolist())
+        have = set(got["col"][got["row"] == kf].tolist())
+        for c_ in want ^ have:
+            assert abs(s_or[c_] - thr[l]) < 1e-3 * thr[l], (h, c_)
+        assert len(want) > 0
+
+
+def test_one_pass_harmonic_sums_errors(torch, fd):
+    with fd.Plan(4096, 20.0, 2.0, 1024, 0) as plan:
+        d_plane = torch.zeros(21, 4096, device="cuda")
+        d_cands = torch.zeros(4 * 16 * 16, dtype=torch.uint8, device="cuda")
+        d_counts = torch.zeros(4, dtype=torch.int64, device="cuda")
+        for levels in ((4, 2), (2, 2), (0, 2), (1, 2, 3, 4, 5)):
+            with pytest.raises(fd.FdasError) as e:
+                plan.harmonic_sums_threshold(None, d_plane, levels, [1.0] * len(levels), d_cands, 16, d_counts)
+            assert e.value.status == 1
+        with pytest.raises(fd.FdasError) as e:
+            plan.harmonic_sums_threshold(None, d_plane, (2, 4), [1.0, float("nan")], d_cands, 16, d_counts)
+        assert e.value.status == 1
+        plan.harmonic_sums_threshold(None, d_plane, (2, 64), [-1.0, -1.0], d_cands, 0, d_counts)   # count only
+        torch.cuda.synchronize()
+        assert d_counts[:2].tolist() == [11 * 2048, 64]           # |z| <= 10: 11 rows x 2048 columns; z = 0 x 64 columns
